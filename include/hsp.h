@@ -1,0 +1,135 @@
+/* hsp.h -- C-ABI boundary of the B200-native Horseshoe-Probit Gibbs sweep.
+ *
+ * Method: Terenin, Dong & Draper, "GPU-accelerated Gibbs sampling: a case study of the Horseshoe
+ * Probit model" (arXiv 1608.04329).  Citations are PAPER.md:<line> (+ section / equation).
+ *
+ * Problem statement the calls follow: inputs are the N x p design matrix X ("the (n x p) matrix
+ * whose rows are the vectors x_i") and y in {0,1}^N; a chain is run
+ * from the cold start beta=0, lambda=nu=tau=xi=1 for n iterations of the sweep
+ * of PAPER.md:188-189 with the full conditionals of eq. (12); the outputs are
+ * the Monte Carlo draws of beta, lambda, tau.
+ *
+ * One sweep (k <- k+1), every step a CUDA kernel of this library (no CPU fallback exists):
+ *   a1  eta_i = x_i . beta
+ *   a2  z_i ~ TN(eta_i, 1) on the side of 0 fixed by y_i
+ *   a3  per-CTA partials of X^T z from the same on-chip tile PAPER.md:200
+ *   b   g = deterministic fixed-order sum of the partials
+ *   e1  lam_j^-2 = -ln u / (nu_j^-1 + tau^-2 beta_j^2 / 2)   PAPER.md:176, 224   (old beta, tau^-2)
+ *   e2  tau^-2 = Gamma((p+1)/2) / (xi^-1 + 1/2 sum lam_j^-2 beta_j^2), Cheng (1977)
+ *   c   Q = X^T X + diag(tau^-2 lam_j^-2)                    PAPER.md:186, 196  (X^T X once, at create)
+ *   d1  Q = L L^T  (blocked fp64 Cholesky)
+ *   d2  beta = Q^-1 g + L^-T e,  e ~ N(0, I)
+ *   e3  nu_j^-1 = -ln u / (1 + lam_j^-2);  xi^-1 = -ln u / (1 + tau^-2)
+ *   g   append beta, lambda_j = (lam_j^-2)^-1/2, tau = (tau^-2)^-1/2 to the device history
+ * Random numbers: Philox-4x32-10, counter (idx_lo, idx_hi, sweep k, tag), key =
+ * seed; one call per variate, so results do not depend on grid shape (DESIGN.md "Random-number
+ * contract").  State, sampler, Gram, Q and L are fp64 whatever the dtype of X.
+ *
+ * Conventions: every call returns an int status (HSP_OK = 0, negative = error), never throws and
+ * never aborts; hsp_last_error() gives a thread-local message for the last failing call.  All
+ * device work is enqueued on the stream given at create; calls that copy results out synchronise
+ * that stream.  "DEVICE" / "HOST" below says where a pointer must live; "ANY" means host or device
+ * (cudaMemcpyDefault).
+ */
+#ifndef HSP_H_
+#define HSP_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hsp_state hsp_state; /* opaque; owned by the library; free with hsp_destroy */
+
+enum { HSP_F32 = 0, HSP_F64 = 1 };
+enum { HSP_OK = 0, HSP_EINVAL = -1, HSP_ENOMEM = -2, HSP_ECUDA = -3, HSP_ENOTPD = -4, HSP_ENUMERIC = -5 };
+/* flags for hsp_set_flags (default: 0) */
+enum {
+  HSP_STORE_Z = 1u,       /* a2 also writes z (fp64, N) to a device buffer for hsp_get_latent      */
+  HSP_FREEZE_SCALES = 2u, /* skip e1, e2, e3 (lambda, tau, nu, xi keep their current values)       */
+  HSP_FREEZE_Z = 4u,      /* skip a1-a3 and b (g keeps the value of the last sweep that ran them)   */
+  HSP_FREEZE_BETA = 16u,  /* skip c, d1, d2 (beta keeps its current value)                          */
+  HSP_NO_GRAPH = 32u,     /* enqueue kernels directly instead of replaying the captured CUDA graph  */
+  HSP_SERIAL = 64u        /* one stream: no overlap of the Cholesky branch with the fused pass      */
+};
+
+/* Create a chain.  PAPER.md:186 (X, y), PAPER.md:289 (cold start), PAPER.md:195 (X^T X once).
+ *   out     HOST   receives the handle (NULL on error).
+ *   X       DEVICE row-major N x p, dtype x_dtype (HSP_F32 | HSP_F64), 16-byte aligned, row pitch
+ *                  p * sizeof(elem).  BORROWED: never copied, never written; the caller keeps it
+ *                  alive until hsp_destroy.
+ *   y       DEVICE N bytes, each 0 or 1.  BORROWED likewise.  Any other value -> HSP_EINVAL.
+ *   N >= 2, p >= 1, seed any 64-bit value.
+ *   stream  cudaStream_t passed as void* (NULL = the legacy default stream).
+ * Runs the Gram kernel (G = X^T X, fp64, exact products) on the stream and returns after it is
+ * enqueued and validated.  Errors: HSP_EINVAL (arguments), HSP_ENOMEM, HSP_ECUDA.               */
+int hsp_create(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N, int p,
+               unsigned long long seed, void* stream);
+
+/* Same, but X and y are HOST buffers (pinned or pageable): the library allocates device copies it
+ * owns, uploads them on the stream (this is the end-to-end entry bench.py times) and frees them in
+ * hsp_destroy.                                                                                   */
+int hsp_create_host(hsp_state** out, const void* X_host, int x_dtype, const unsigned char* y_host,
+                    long long N, int p, unsigned long long seed, void* stream);
+
+/* Run n_iter sweeps (steps a1..g above, in the order PAPER.md:188-189 fixes), asynchronously on the
+ * stream.  The draws of this call replace the history of the previous call.  n_iter >= 0.
+ * Errors: HSP_EINVAL, HSP_ENOMEM (history n_iter*(2p+1)*8 bytes), HSP_ECUDA.  A Cholesky breakdown
+ * or non-finite state inside the sweeps is reported by the next synchronising call
+ * (hsp_get_draws / hsp_get_state / hsp_sync) as HSP_ENOTPD / HSP_ENUMERIC.                       */
+int hsp_sweep(hsp_state* s, long long n_iter);
+
+/* Copy the draws of the most recent hsp_sweep call: beta[n_iter*p],
+ * lambda[n_iter*p], tau[n_iter], row-major by sweep.  ANY pointers; any may be NULL.
+ * Synchronises the stream.                                                                       */
+int hsp_get_draws(const hsp_state* s, double* beta, double* lambda, double* tau);
+
+/* Synchronise the stream and report device-side status (HSP_OK, HSP_ENOTPD, HSP_ENUMERIC).       */
+int hsp_sync(const hsp_state* s);
+
+int hsp_destroy(hsp_state* s);
+
+/* Thread-local message of the last call that failed on this thread ("" if none).                 */
+const char* hsp_last_error(void);
+
+/* ---- debug / test / measurement entry points ------------------------------------------------ */
+
+/* z of the last sweep (needs HSP_STORE_Z set before that sweep, else HSP_EINVAL) and the truncation
+ * side 2y-1.  ANY pointers, may be NULL.  Synchronises.                           */
+int hsp_get_latent(const hsp_state* s, double* z, signed char* side);
+/* Current state; p-vectors and scalars, ANY pointers, may be NULL.  sweep = number of sweeps done. */
+int hsp_get_state(const hsp_state* s, double* beta, double* lam_inv2, double* nu_inv, double* tau_inv2,
+                  double* xi_inv, long long* sweep);
+/* Overwrite parts of the state (NULL = keep; sweep < 0 = keep).  Because the random numbers are a
+ * pure function of (seed, index, sweep, tag), get_state/set_state give exact checkpoint/resume.   */
+int hsp_set_state(hsp_state* s, const double* beta, const double* lam_inv2, const double* nu_inv,
+                  const double* tau_inv2, const double* xi_inv, long long sweep);
+int hsp_set_flags(hsp_state* s, unsigned flags);
+/* g = X^T z of the last sweep (p), G = X^T X (p*p, row-major, lower triangle valid), L (p*p, lower). */
+int hsp_get_xtz(const hsp_state* s, double* g);
+int hsp_get_gram(const hsp_state* s, double* G);
+int hsp_get_chol(const hsp_state* s, double* L);
+/* Average device time (ms) of the fused pass a1-a3 over the launches since the last call of this
+ * function, measured with CUDA events on the launching stream when HSP_NO_GRAPH is set; and the
+ * number of launches averaged.  Synchronises.                                                    */
+int hsp_get_fused_pass_ms(hsp_state* s, double* ms, long long* launches);
+/* Number of kernels this library launched (directly or through graph replays) since create.      */
+long long hsp_get_launch_count(const hsp_state* s);
+/* Name of the fused-pass kernel variant selected for this (dtype, p): "tma" or "generic".        */
+const char* hsp_fused_variant(const hsp_state* s);
+
+/* Device unit-test hooks (one thread per element; DEVICE pointers):
+ *   philox : out[4n] = Philox-4x32-10(ctr[4n], key[2n])
+ *   uniform: ua[n], ub[n] from (seed, idx[n], sweep, tag) -- the variate addressing of the sweep
+ *   tnpos  : w[n] = TNpos(m[n], u[n]);   norm_inv: x[n] = Phi^-1(u[n])
+ *   cheng  : x[n] = Gamma(alpha, 1) drawn with (seed, sweep = sweep0 + i)                         */
+int hsp_dbg_philox(const unsigned* ctr, const unsigned* key, unsigned* out, long long n, void* stream);
+int hsp_dbg_uniform(unsigned long long seed, const unsigned long long* idx, unsigned sweep, unsigned tag,
+                    double* ua, double* ub, long long n, void* stream);
+int hsp_dbg_tnpos(const double* m, const double* u, double* w, long long n, void* stream);
+int hsp_dbg_norm_inv(const double* u, double* x, long long n, void* stream);
+int hsp_dbg_cheng(double alpha, unsigned long long seed, unsigned sweep0, double* x, long long n, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HSP_H_ */

@@ -24,6 +24,12 @@ def lib():
         for name in ("hspo_qinv", "hspo_norm_inv"):
             getattr(L, name).argtypes = [C.c_double]
             getattr(L, name).restype = C.c_double
+        L.hspo_philox_many.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]
+        L.hspo_philox_many.restype = None
+        L.hspo_uniforms_many.argtypes = [C.c_uint64, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p, C.c_longlong]
+        L.hspo_uniforms_many.restype = None
+        L.hspo_norm_inv_many.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong]
+        L.hspo_norm_inv_many.restype = None
         L.hspo_tnpos.argtypes = [C.c_double, C.c_double]
         L.hspo_tnpos.restype = C.c_double
         L.hspo_tnpos_many.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]
@@ -77,6 +83,28 @@ def uniforms(seed, idx, sweep, tag):
     a, b = C.c_double(), C.c_double()
     lib().hspo_uniforms(seed, idx, sweep, tag, C.byref(a), C.byref(b))
     return a.value, b.value
+
+
+def philox_many(ctr, key):
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32)
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.empty_like(ctr)
+    lib().hspo_philox_many(_ptr(ctr), _ptr(key), _ptr(out), ctr.shape[0])
+    return out
+
+
+def uniforms_many(seed, idx, sweep, tag):
+    idx = np.ascontiguousarray(idx, dtype=np.uint64)
+    ua, ub = np.empty(idx.size), np.empty(idx.size)
+    lib().hspo_uniforms_many(seed, _ptr(idx), sweep, tag, _ptr(ua), _ptr(ub), idx.size)
+    return ua, ub
+
+
+def norm_inv_many(u):
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    x = np.empty_like(u)
+    lib().hspo_norm_inv_many(_ptr(u), _ptr(x), u.size)
+    return x
 
 
 def qinv(q):

@@ -356,6 +356,13 @@ extern "C" {
 
 void hspo_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
 void hspo_uniforms(uint64_t seed, uint64_t idx, uint32_t sweep, uint32_t tag, double* ua, double* ub) { uniforms(seed, idx, sweep, tag, ua, ub); }
+void hspo_philox_many(const uint32_t* ctr, const uint32_t* key, uint32_t* out, long long n) {
+  for (long long i = 0; i < n; ++i) philox4x32_10(ctr + 4 * i, key + 2 * i, out + 4 * i);
+}
+void hspo_uniforms_many(uint64_t seed, const uint64_t* idx, uint32_t sweep, uint32_t tag, double* ua, double* ub, long long n) {
+  for (long long i = 0; i < n; ++i) uniforms(seed, idx[i], sweep, tag, ua ? ua + i : nullptr, ub ? ub + i : nullptr);
+}
+void hspo_norm_inv_many(const double* u, double* x, long long n) { for (long long i = 0; i < n; ++i) x[i] = norm_inv(u[i]); }
 double hspo_qinv(double q) { return q <= 0.5 ? (double)qinv_half(q) : (double)(-qinv_half(1.0L - (long double)q)); }
 double hspo_norm_inv(double u) { return norm_inv(u); }
 double hspo_tnpos(double m, double u) { return tnpos(m, u); }

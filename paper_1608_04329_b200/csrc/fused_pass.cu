@@ -1,0 +1,517 @@
+// fused_pass.cu -- rows a1, a2, a3 and b of the hot path (include/hsp.h):
+//   one streaming pass over X that computes eta_i = x_i.beta, draws
+//   z_i ~ TN(eta_i,1) on the side fixed by y_i and accumulates X^T z
+//    from the same on-chip tile, so X is read from HBM once per sweep; then a
+//   fixed-order reduction of the per-CTA partials.
+//
+// Two kernels:
+//   fused_pass_tma     persistent, warp-specialised: one producer thread streams row tiles with
+//                      cp.async.bulk (TMA, 1-D: a tile of R rows is contiguous in row-major X) into
+//                      an S-stage shared-memory ring guarded by mbarriers; 8 compute warps own
+//                      fixed column stripes (eta partials -> shuffle reduce -> smem; later, x*z
+//                      accumulation from the same stage); 4 sampler warps turn eta into z (Philox +
+//                      inverse-CDF) D tiles behind the eta phase, so the sampler's latency is hidden
+//                      behind the stream.  Static tile->CTA map: bit-reproducible run to run.
+//   fused_pass_generic any p, any alignment (rows not a multiple of 16 bytes, or narrow p):
+//                      thread-per-row eta + sampler, then thread-per-column accumulation that
+//                      re-reads the 256-row tile from L1/L2.
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdlib>
+#include <cstdio>
+#include "hsp_device.cuh"
+#include "hsp_internal.h"
+
+namespace hsp {
+
+// ------------------------------------------------------------------------------------------------
+// PTX helpers (mbarrier + 1-D bulk copy)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred P1;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+      "@P1 bra DONE;\n\t"
+      "bra WAIT_LOOP;\n\t"
+      "DONE:\n\t"
+      "}" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+      "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// Column-stripe arithmetic for one 16-byte vector of X
+// ------------------------------------------------------------------------------------------------
+template <typename XT> struct Vec;
+template <> struct Vec<float> {
+  static constexpr int V = 4;
+  using Acc = float;
+  float4 v;
+  __device__ __forceinline__ void load(const unsigned char* smem) { v = *reinterpret_cast<const float4*>(smem); }
+  __device__ __forceinline__ double dot(const double* b) const {
+    double s = (double)v.x * b[0];
+    s = fma((double)v.y, b[1], s);
+    s = fma((double)v.z, b[2], s);
+    s = fma((double)v.w, b[3], s);
+    return s;
+  }
+  __device__ __forceinline__ void axpy(float z, float* acc) const {
+    acc[0] = fmaf(v.x, z, acc[0]);
+    acc[1] = fmaf(v.y, z, acc[1]);
+    acc[2] = fmaf(v.z, z, acc[2]);
+    acc[3] = fmaf(v.w, z, acc[3]);
+  }
+};
+template <> struct Vec<double> {
+  static constexpr int V = 2;
+  using Acc = double;
+  double2 v;
+  __device__ __forceinline__ void load(const unsigned char* smem) { v = *reinterpret_cast<const double2*>(smem); }
+  __device__ __forceinline__ double dot(const double* b) const { return fma(v.y, b[1], v.x * b[0]); }
+  __device__ __forceinline__ void axpy(double z, double* acc) const {
+    acc[0] = fma(v.x, z, acc[0]);
+    acc[1] = fma(v.y, z, acc[1]);
+  }
+};
+
+// Reduce RT per-lane values over the 32 lanes of a warp with a fixed butterfly; on return v[0] of
+// lane l is the warp total of row rows_of_lane<RT>(l).  (RT + 4..5 shuffles instead of 5 RT.)
+template <int RT>
+__device__ __forceinline__ double warp_reduce_rows(double (&v)[RT], int lane) {
+  int off = 16;
+#pragma unroll
+  for (int n = RT; n > 1; n >>= 1, off >>= 1) {
+    const bool upper = (lane & off) != 0;
+#pragma unroll
+    for (int i = 0; i < n / 2; ++i) {
+      const double send = upper ? v[i] : v[i + n / 2];
+      const double keep = upper ? v[i + n / 2] : v[i];
+      v[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+    }
+  }
+  for (; off >= 1; off >>= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], off);
+  return v[0];
+}
+template <int RT>
+__device__ __forceinline__ int row_of_lane(int lane) {
+  int row = 0, off = 16;
+#pragma unroll
+  for (int n = RT; n > 1; n >>= 1, off >>= 1) row += (lane & off) ? n / 2 : 0;
+  return row;
+}
+
+constexpr int kComputeWarps = 8;
+constexpr int kComputeThreads = kComputeWarps * 32;
+constexpr int kSamplerWarps = 4;
+constexpr int kTmaThreads = (kComputeWarps + kSamplerWarps + 1) * 32;
+constexpr int kFlushRows = 16;   // fp32 x*z chains are flushed into the fp64 accumulators every >= 16 rows
+
+struct TmaSmemLayout {
+  size_t tiles, eta_part, z64, z32, bars, total;
+  __host__ __device__ TmaSmemLayout(int S, int R, size_t stage_bytes) {
+    tiles = 0;
+    eta_part = tiles + (size_t)S * stage_bytes;
+    z64 = eta_part + (size_t)S * kComputeWarps * R * sizeof(double);
+    z32 = z64 + (size_t)S * R * sizeof(double);
+    bars = (z32 + (size_t)S * R * sizeof(float) + 15) & ~(size_t)15;
+    total = bars + (size_t)4 * S * sizeof(uint64_t);
+  }
+};
+
+template <typename XT, int RT, int C>
+__global__ void __launch_bounds__(kTmaThreads, 1)
+fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
+               unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
+               double* __restrict__ partial, double* __restrict__ z_out, int S, int D, long long n_tiles) {
+  constexpr int V = Vec<XT>::V;
+  using Acc = typename Vec<XT>::Acc;
+  constexpr bool kF32 = sizeof(XT) == 4;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const size_t row_bytes = (size_t)p * sizeof(XT);
+  const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
+  const TmaSmemLayout lay(S, RT, stage_bytes);
+  unsigned char* tiles = smem + lay.tiles;
+  double* eta_part = reinterpret_cast<double*>(smem + lay.eta_part);
+  double* z64 = reinterpret_cast<double*>(smem + lay.z64);
+  float* z32 = reinterpret_cast<float*>(smem + lay.z32);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + lay.bars);
+  uint64_t* empty = full + S;
+  uint64_t* eta_full = empty + S;
+  uint64_t* z_full = eta_full + S;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const long long cta = blockIdx.x, grid = gridDim.x;
+  const long long my_tiles = cta < n_tiles ? (n_tiles - cta + grid - 1) / grid : 0;
+  const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
+
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], kComputeWarps);
+      mbar_init(&eta_full[s], kComputeWarps);
+      mbar_init(&z_full[s], 1);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp == kComputeWarps + kSamplerWarps) {
+    // ===================== producer: one thread streams the tiles =====================
+    if (lane == 0) {
+      for (long long n = 0; n < my_tiles; ++n) {
+        const int st = (int)(n % S);
+        const uint32_t ph = (uint32_t)((n / S) & 1);
+        mbar_wait(&empty[st], ph ^ 1u);
+        const long long row0 = (cta + n * grid) * RT;
+        const long long rows = (N - row0) < RT ? (N - row0) : RT;
+        const uint32_t bytes = (uint32_t)((size_t)rows * row_bytes);
+        mbar_arrive_expect_tx(&full[st], bytes);
+        bulk_g2s(tiles + (size_t)st * stage_bytes, reinterpret_cast<const unsigned char*>(X) + (size_t)row0 * row_bytes,
+                 bytes, &full[st]);
+      }
+    }
+  } else if (warp >= kComputeWarps) {
+    // ===================== sampler warps: eta -> z, D tiles behind the eta phase =====================
+    const int sw = warp - kComputeWarps;
+    for (long long n = sw; n < my_tiles; n += kSamplerWarps) {
+      const int st = (int)(n % S);
+      const uint32_t ph = (uint32_t)((n / S) & 1);
+      const long long row0 = (cta + n * grid) * RT;
+      // everything that does not depend on eta first: y, the Philox uniform
+      const long long i = row0 + lane;
+      const bool valid = (lane < RT) && (i < N);
+      const double ystar = valid ? 2.0 * (double)y[i] - 1.0 : 1.0;
+      const double u = uniform_a(seed, (unsigned long long)(valid ? i : 0), sweep, TAG_Z);
+      mbar_wait(&eta_full[st], ph);
+      double eta = 0.0;
+      if (lane < RT) {
+#pragma unroll
+        for (int w = 0; w < kComputeWarps; ++w) eta += eta_part[((size_t)st * kComputeWarps + w) * RT + lane];
+      }
+      const double wpos = tnpos(ystar * eta, u);
+      const double z = valid ? ystar * wpos : 0.0;
+      if (lane < RT) {
+        z64[st * RT + lane] = z;
+        z32[st * RT + lane] = (float)z;
+      }
+      if (valid && z_out != nullptr) z_out[i] = z;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&z_full[st]);
+    }
+  } else {
+    // ===================== compute warps: eta partials, then x*z from the same stage =====================
+    double breg[C][V];
+    double acc64[C][V];
+    Acc acc[C][V];
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      const int col = (c * kComputeThreads + tid) * V;
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        breg[c][v] = (col + v < p) ? beta[col + v] : 0.0;
+        acc64[c][v] = 0.0;
+        acc[c][v] = (Acc)0;
+      }
+    }
+    const int my_row = row_of_lane<RT>(lane);
+    const bool writer = (lane & (32 / RT - 1)) == 0;
+    int rows_since_flush = 0;
+    for (long long it = 0; it < my_tiles + D; ++it) {
+      if (it < my_tiles) {
+        const int st = (int)(it % S);
+        const uint32_t ph = (uint32_t)((it / S) & 1);
+        mbar_wait(&full[st], ph);
+        const unsigned char* tile = tiles + (size_t)st * stage_bytes;
+        double part[RT];
+#pragma unroll
+        for (int r = 0; r < RT; ++r) part[r] = 0.0;
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+          const int col = (c * kComputeThreads + tid) * V;
+          if (col < p) {
+#pragma unroll
+            for (int r = 0; r < RT; ++r) {
+              Vec<XT> x;
+              x.load(tile + (size_t)r * row_bytes + (size_t)col * sizeof(XT));
+              part[r] += x.dot(breg[c]);
+            }
+          }
+        }
+        const double tot = warp_reduce_rows<RT>(part, lane);
+        if (writer) eta_part[((size_t)st * kComputeWarps + warp) * RT + my_row] = tot;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&eta_full[st]);
+      }
+      if (it >= D) {
+        const long long n2 = it - D;
+        const int st = (int)(n2 % S);
+        const uint32_t ph = (uint32_t)((n2 / S) & 1);
+        mbar_wait(&z_full[st], ph);
+        const unsigned char* tile = tiles + (size_t)st * stage_bytes;
+        const long long row0 = (cta + n2 * grid) * RT;
+        const int nrows = (N - row0) < RT ? (int)(N - row0) : RT;
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+          if (r < nrows) {
+            Acc zr;
+            if constexpr (kF32) zr = z32[st * RT + r]; else zr = z64[st * RT + r];
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+              const int col = (c * kComputeThreads + tid) * V;
+              if (col < p) {
+                Vec<XT> x;
+                x.load(tile + (size_t)r * row_bytes + (size_t)col * sizeof(XT));
+                x.axpy(zr, acc[c]);
+              }
+            }
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[st]);
+        if constexpr (kF32) {
+          rows_since_flush += RT;
+          if (rows_since_flush >= kFlushRows) {
+            rows_since_flush = 0;
+#pragma unroll
+            for (int c = 0; c < C; ++c)
+#pragma unroll
+              for (int v = 0; v < V; ++v) { acc64[c][v] += (double)acc[c][v]; acc[c][v] = (Acc)0; }
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      const int col = (c * kComputeThreads + tid) * V;
+#pragma unroll
+      for (int v = 0; v < V; ++v)
+        if (col + v < p) partial[(size_t)cta * p + col + v] = acc64[c][v] + (double)acc[c][v];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Generic kernel: any p / alignment.  256-row tiles; phase 1 thread-per-row, phase 2 thread-per-column.
+// ------------------------------------------------------------------------------------------------
+constexpr int kGenThreads = 256;
+constexpr int kGenMaxC = 16;
+
+template <typename XT>
+__global__ void __launch_bounds__(kGenThreads)
+fused_pass_generic(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
+                   unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
+                   double* __restrict__ partial, double* __restrict__ z_out, int csg /*pow2 column slots*/) {
+  __shared__ double z_s[kGenThreads];
+  __shared__ double red[kGenThreads];
+  const int tid = threadIdx.x;
+  const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
+  const int rg_count = kGenThreads / csg, rg = tid / csg, cs = tid % csg;
+  const int C = (p + csg - 1) / csg;                 // column chunks per thread (1 when csg < 256)
+  const bool in_regs = C <= kGenMaxC;
+  double acc[kGenMaxC];
+#pragma unroll
+  for (int c = 0; c < kGenMaxC; ++c) acc[c] = 0.0;
+  double* my_partial = partial + (size_t)blockIdx.x * p;
+  if (!in_regs)
+    for (int j = tid; j < p; j += kGenThreads) my_partial[j] = 0.0;
+  const long long n_tiles = (N + kGenThreads - 1) / kGenThreads;
+  for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+    const long long row0 = t * kGenThreads;
+    const long long i = row0 + tid;
+    double z = 0.0;
+    if (i < N) {
+      const XT* xr = X + (size_t)i * p;
+      double eta = 0.0;
+      for (int j = 0; j < p; ++j) eta = fma((double)xr[j], beta[j], eta);
+      const double ystar = 2.0 * (double)y[i] - 1.0;
+      const double u = uniform_a(seed, (unsigned long long)i, sweep, TAG_Z);
+      z = ystar * tnpos(ystar * eta, u);
+      if (z_out != nullptr) z_out[i] = z;
+    }
+    __syncthreads();     // previous tile's phase 2 is done with z_s
+    z_s[tid] = z;
+    __syncthreads();
+    const int nrows = (N - row0) < kGenThreads ? (int)(N - row0) : kGenThreads;
+    if (in_regs) {
+#pragma unroll
+      for (int c = 0; c < kGenMaxC; ++c) {
+        const int j = c * csg + cs;
+        if (c < C && j < p) {
+          double a = 0.0;
+          for (int r = rg; r < nrows; r += rg_count) a = fma((double)X[(size_t)(row0 + r) * p + j], z_s[r], a);
+          acc[c] += a;
+        }
+      }
+    } else {
+      for (int j = tid; j < p; j += kGenThreads) {
+        double a = 0.0;
+        for (int r = 0; r < nrows; ++r) a = fma((double)X[(size_t)(row0 + r) * p + j], z_s[r], a);
+        my_partial[j] += a;
+      }
+    }
+  }
+  if (in_regs) {
+    if (rg_count == 1) {
+#pragma unroll
+      for (int c = 0; c < kGenMaxC; ++c) {
+        const int j = c * csg + cs;
+        if (c < C && j < p) my_partial[j] = acc[c];
+      }
+    } else {   // C == 1: combine the row groups in fixed order
+      __syncthreads();
+      red[tid] = acc[0];
+      __syncthreads();
+      if (rg == 0 && cs < p) {
+        double s = 0.0;
+        for (int q = 0; q < rg_count; ++q) s += red[q * csg + cs];
+        my_partial[cs] = s;
+      }
+    }
+  }
+}
+
+// b: g_j = sum_c partial[c][j], c ascending (no float atomics)
+__global__ void reduce_partials_kernel(const double* __restrict__ partial, int n_part, int p, double* __restrict__ g) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= p) return;
+  double s = 0.0;
+  for (int c = 0; c < n_part; ++c) s += partial[(size_t)c * p + j];
+  g[j] = s;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host side: variant selection and launch
+// ------------------------------------------------------------------------------------------------
+static int env_int(const char* name, int dflt) {
+  const char* v = getenv(name);
+  return (v && *v) ? atoi(v) : dflt;
+}
+
+static int round_chunks(int c) {
+  const int opts[] = {1, 2, 3, 4, 6, 8, 12, 16};
+  for (int o : opts) if (c <= o) return o;
+  return 0;
+}
+static int rows_for_chunks(int c) { return c == 1 ? 8 : c == 2 ? 4 : c <= 4 ? 2 : 1; }
+
+FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X) {
+  FusedPlan pl{};
+  const size_t elem = dtype == kF32 ? 4 : 8;
+  const int V = (int)(16 / elem);
+  const size_t row_bytes = (size_t)p * elem;
+  const int c_raw = (int)((p + V * kComputeThreads - 1) / (V * kComputeThreads));
+  const int C = round_chunks(c_raw);
+  const bool aligned = (row_bytes % 16 == 0) && ((reinterpret_cast<uintptr_t>(X) & 15) == 0);
+  const bool wide = (p / V) >= kComputeThreads / 2;
+  const int force = env_int("HSP_FUSED_VARIANT", -1);
+  if (aligned && C != 0 && (wide || force == 1) && force != 0) {
+    const int RT = rows_for_chunks(C);
+    const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
+    const size_t budget = 227 * 1024;
+    int S = env_int("HSP_FUSED_STAGES", 0);
+    if (S <= 0) {
+      S = 12;
+      while (S > 2 && TmaSmemLayout(S, RT, stage_bytes).total > budget) --S;
+    }
+    if (S >= 3 && TmaSmemLayout(S, RT, stage_bytes).total <= budget) {
+      int D = env_int("HSP_FUSED_LAG", 0);
+      if (D <= 0) D = (S - 1) / 2;
+      if (D > S - 2) D = S - 2;
+      if (D < 1) D = 1;
+      pl.variant = 1;
+      pl.rows_per_tile = RT; pl.chunks = C; pl.stages = S; pl.lag = D;
+      pl.n_tiles = (N + RT - 1) / RT;
+      int grid = env_int("HSP_FUSED_GRID", num_sms);
+      if ((long long)grid > pl.n_tiles) grid = (int)pl.n_tiles;
+      pl.grid = grid; pl.block = kTmaThreads;
+      pl.smem = TmaSmemLayout(S, RT, stage_bytes).total;
+      return pl;
+    }
+  }
+  pl.variant = 0;
+  pl.n_tiles = (N + kGenThreads - 1) / kGenThreads;
+  long long grid = (long long)num_sms * 4;
+  if (grid > pl.n_tiles) grid = pl.n_tiles;
+  pl.grid = (int)grid; pl.block = kGenThreads; pl.smem = 0;
+  pl.rows_per_tile = kGenThreads; pl.chunks = 0; pl.stages = 0; pl.lag = 0;
+  return pl;
+}
+
+template <typename XT, int RT, int C>
+static cudaError_t launch_tma(const FusedPlan& pl, const void* X, const unsigned char* y, long long N, int p,
+                              unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
+                              double* z_out, cudaStream_t st) {
+  auto kern = fused_pass_tma<XT, RT, C>;
+  static bool configured = false;   // per instantiation
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  if (N < 0) return cudaSuccess;     // prepare-only call (sets the attribute outside stream capture)
+  kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
+                                          pl.stages, pl.lag, pl.n_tiles);
+  return cudaGetLastError();
+}
+
+template <typename XT>
+static cudaError_t dispatch_tma(const FusedPlan& pl, const void* X, const unsigned char* y, long long N, int p,
+                                unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
+                                double* z_out, cudaStream_t st) {
+  switch (pl.chunks) {
+    case 1: return launch_tma<XT, 8, 1>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+    case 2: return launch_tma<XT, 4, 2>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+    case 3: return launch_tma<XT, 2, 3>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+    case 4: return launch_tma<XT, 2, 4>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+    case 6: return launch_tma<XT, 1, 6>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+    case 8: return launch_tma<XT, 1, 8>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+    case 12: return launch_tma<XT, 1, 12>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+    case 16: return launch_tma<XT, 1, 16>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+  }
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t fused_pass_launch(const FusedPlan& pl, const void* X, int dtype, const unsigned char* y, long long N,
+                              int p, unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
+                              double* z_out, cudaStream_t st) {
+  if (pl.variant != 1 && N < 0) return cudaSuccess;
+  if (pl.variant == 1) {
+    return dtype == kF32 ? dispatch_tma<float>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st)
+                         : dispatch_tma<double>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+  }
+  int csg = 1;
+  while (csg < p && csg < kGenThreads) csg <<= 1;
+  if (dtype == kF32)
+    fused_pass_generic<float><<<pl.grid, pl.block, 0, st>>>(static_cast<const float*>(X), y, N, p, seed, beta, ctl,
+                                                            partial, z_out, csg);
+  else
+    fused_pass_generic<double><<<pl.grid, pl.block, 0, st>>>(static_cast<const double*>(X), y, N, p, seed, beta, ctl,
+                                                             partial, z_out, csg);
+  return cudaGetLastError();
+}
+
+cudaError_t reduce_partials_launch(const double* partial, int n_part, int p, double* g, cudaStream_t st) {
+  reduce_partials_kernel<<<(p + 127) / 128, 128, 0, st>>>(partial, n_part, p, g);
+  return cudaGetLastError();
+}
+
+}  // namespace hsp

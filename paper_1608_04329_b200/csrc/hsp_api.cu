@@ -1,0 +1,485 @@
+// hsp_api.cu -- the C-ABI boundary (include/hsp.h) and the host orchestrator of the sweep.
+//
+// Sweep DAG:   {a1 a2 a3 -> b}  ||  {e1 e2 -> c -> d1}  ->  d2 -> e3, g
+// The Cholesky branch depends only on the previous beta, so it runs on a second stream beside the
+// fused pass; one sweep is captured into a CUDA graph and replayed n_iter times (all kernel
+// arguments that change between sweeps live in the device control block Ctl).
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+#include <new>
+#include "../../include/hsp.h"
+#include "hsp_device.cuh"
+#include "hsp_internal.h"
+
+using namespace hsp;
+
+static thread_local std::string g_err;
+static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+static int cuda_fail(cudaError_t e, const char* what) {
+  g_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return e == cudaErrorMemoryAllocation ? HSP_ENOMEM : HSP_ECUDA;
+}
+#define CK(call)                                   \
+  do {                                             \
+    cudaError_t e_ = (call);                       \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+struct hsp_state {
+  const void* X = nullptr; int dtype = 0; const unsigned char* y = nullptr; long long N = 0; int p = 0;
+  unsigned long long seed = 0; cudaStream_t stream = nullptr; cudaStream_t stream2 = nullptr;
+  cudaStream_t own_stream = nullptr;
+  unsigned flags = 0; int num_sms = 0;
+  void* own_X = nullptr; unsigned char* own_y = nullptr;
+  double *G = nullptr, *L = nullptr, *beta = nullptr, *lam_inv2 = nullptr, *nu_inv = nullptr, *g = nullptr,
+         *partial = nullptr, *z = nullptr;
+  signed char* side = nullptr;
+  Ctl* ctl = nullptr;
+  double *h_beta = nullptr, *h_lambda = nullptr, *h_tau = nullptr;
+  long long h_cap = 0, h_n = 0, host_sweep = 0;
+  bool z_valid = false;
+  FusedPlan plan{};
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  cudaGraphExec_t graph_exec = nullptr; unsigned graph_flags = ~0u; long long graph_kernels = 0;
+  long long launches = 0;
+  std::vector<cudaEvent_t> tev;   // event pairs around the fused pass (direct-launch mode)
+  size_t tev_used = 0; double fused_ms_sum = 0.0; long long fused_n = 0;
+};
+
+static void free_state(hsp_state* s) {
+  if (!s) return;
+  if (s->graph_exec) cudaGraphExecDestroy(s->graph_exec);
+  for (cudaEvent_t e : s->tev) cudaEventDestroy(e);
+  if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+  if (s->ev_join) cudaEventDestroy(s->ev_join);
+  if (s->stream2) cudaStreamDestroy(s->stream2);
+  if (s->own_stream) cudaStreamDestroy(s->own_stream);
+  void* ptrs[] = {s->own_X, s->own_y, s->G, s->L, s->beta, s->lam_inv2, s->nu_inv, s->g, s->partial, s->z, s->side,
+                  s->ctl, s->h_beta, s->h_lambda, s->h_tau};
+  for (void* q : ptrs) if (q) cudaFree(q);
+  delete s;
+}
+
+static int drain_fused_events(hsp_state* s) {
+  for (size_t i = 0; i + 1 < s->tev_used; i += 2) {
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, s->tev[i], s->tev[i + 1]));
+    s->fused_ms_sum += ms; s->fused_n += 1;
+  }
+  s->tev_used = 0;
+  return HSP_OK;
+}
+
+// Enqueue one sweep.  `timed`: bracket the fused pass with CUDA events (direct-launch mode only).
+static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
+  cudaStream_t A = s->stream;
+  const bool serial = (s->flags & HSP_SERIAL) != 0;
+  cudaStream_t B = serial ? A : s->stream2;
+  const bool do_z = !(s->flags & HSP_FREEZE_Z), do_scales = !(s->flags & HSP_FREEZE_SCALES),
+             do_beta = !(s->flags & HSP_FREEZE_BETA);
+  const bool side_work = do_scales || do_beta;
+  if (!serial && side_work) {
+    CK(cudaEventRecord(s->ev_fork, A));
+    CK(cudaStreamWaitEvent(B, s->ev_fork, 0));
+  }
+  if (do_z) {
+    if (timed) {
+      if (s->tev_used + 2 > s->tev.size()) {
+        for (int q = 0; q < 2; ++q) { cudaEvent_t e; CK(cudaEventCreate(&e)); s->tev.push_back(e); }
+      }
+      CK(cudaEventRecord(s->tev[s->tev_used], A));
+    }
+    CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, s->N, s->p, s->seed, s->beta, s->ctl, s->partial,
+                         (s->flags & HSP_STORE_Z) ? s->z : nullptr, A));
+    if (timed) { CK(cudaEventRecord(s->tev[s->tev_used + 1], A)); s->tev_used += 2; }
+    CK(reduce_partials_launch(s->partial, s->plan.grid, s->p, s->g, A));
+    *kernels += 2;
+  }
+  if (do_scales) { CK(scales_pre_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, B)); *kernels += 1; }
+  if (do_beta) {
+    CK(build_q_launch(s->G, s->lam_inv2, s->ctl, s->L, s->p, B)); *kernels += 1;
+    CK(cholesky_launch(s->L, s->p, s->ctl, B, kernels));
+  }
+  if (!serial && side_work) {
+    CK(cudaEventRecord(s->ev_join, B));
+    CK(cudaStreamWaitEvent(A, s->ev_join, 0));
+  }
+  if (do_beta) { CK(beta_draw_launch(s->L, s->g, s->beta, s->p, s->seed, s->ctl, A)); *kernels += 1; }
+  CK(scales_post_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, do_scales ? 0 : 1, A));
+  *kernels += 1;
+  return HSP_OK;
+}
+
+static int build_graph(hsp_state* s) {
+  if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+  cudaGraph_t graph = nullptr;
+  CK(cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+  long long kernels = 0;
+  const int rc = enqueue_sweep(s, false, &kernels);
+  cudaError_t e = cudaStreamEndCapture(s->stream, &graph);
+  if (rc != HSP_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+  if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+  e = cudaGraphInstantiate(&s->graph_exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate");
+  s->graph_flags = s->flags; s->graph_kernels = kernels;
+  return HSP_OK;
+}
+
+static int create_common(hsp_state** out, hsp_state* s) {
+  const int p = s->p; const long long N = s->N;
+  int dev = 0;
+  CK(cudaGetDevice(&dev));
+  if (s->stream == nullptr) {
+    // the legacy default stream cannot be captured into a graph: use a blocking stream of our own,
+    // which still orders itself after/before work on the legacy stream
+    CK(cudaStreamCreateWithFlags(&s->own_stream, cudaStreamDefault));
+    s->stream = s->own_stream;
+  }
+  CK(cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev));
+  CK(cudaStreamCreateWithFlags(&s->stream2, cudaStreamNonBlocking));
+  CK(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
+  CK(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
+  s->plan = fused_plan(s->dtype, N, p, s->num_sms, s->X);
+  // set opt-in shared-memory attributes now, outside any stream capture
+  CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, -1, p, 0, nullptr, nullptr, nullptr, nullptr, s->stream));
+  CK(beta_draw_launch(nullptr, nullptr, nullptr, p, 0, nullptr, s->stream));
+  const size_t pp = (size_t)p * p * sizeof(double), pv = (size_t)p * sizeof(double);
+  CK(cudaMalloc(&s->G, pp)); CK(cudaMalloc(&s->L, pp));
+  CK(cudaMalloc(&s->beta, pv)); CK(cudaMalloc(&s->lam_inv2, pv)); CK(cudaMalloc(&s->nu_inv, pv)); CK(cudaMalloc(&s->g, pv));
+  CK(cudaMalloc(&s->partial, (size_t)s->plan.grid * pv));
+  CK(cudaMalloc(&s->ctl, sizeof(Ctl)));
+  // validate y in {0,1}
+  int* bad = nullptr;
+  CK(cudaMalloc(&bad, sizeof(int)));
+  CK(cudaMemsetAsync(bad, 0, sizeof(int), s->stream));
+  CK(validate_y_launch(s->y, N, bad, s->stream));
+  int h_bad = 0;
+  CK(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  cudaFree(bad);
+  s->launches += 1;
+  if (h_bad) return fail(HSP_EINVAL, "y must contain only 0 and 1");
+  // cold start: beta = 0; lambda = nu = tau = xi = 1
+  std::vector<double> ones((size_t)p, 1.0);
+  CK(cudaMemsetAsync(s->beta, 0, pv, s->stream));
+  CK(cudaMemsetAsync(s->g, 0, pv, s->stream));
+  CK(cudaMemcpyAsync(s->lam_inv2, ones.data(), pv, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->nu_inv, ones.data(), pv, cudaMemcpyHostToDevice, s->stream));
+  Ctl c{}; c.sweep = 0; c.hist_base = 0; c.tau_inv2 = 1.0; c.xi_inv = 1.0; c.status = 0;
+  c.h_beta = c.h_lambda = c.h_tau = nullptr;
+  CK(cudaMemcpyAsync(s->ctl, &c, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaStreamSynchronize(s->stream));   // `ones` and `c` are stack/heap temporaries
+  // c0: G = X^T X once
+  const int splits = gram_splits(N, p, s->num_sms);
+  double* scratch = s->L;                  // L is free until the first sweep
+  if (splits > 1) CK(cudaMalloc(&scratch, (size_t)splits * pp));
+  cudaError_t e = gram_launch(s->X, s->dtype, N, p, s->G, scratch, splits, s->stream);
+  s->launches += 3;
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (splits > 1) cudaFree(scratch);
+  if (e != cudaSuccess) return cuda_fail(e, "gram");
+  *out = s;
+  return HSP_OK;
+}
+
+extern "C" {
+
+const char* hsp_last_error(void) { return g_err.c_str(); }
+
+int hsp_create(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N, int p,
+               unsigned long long seed, void* stream) {
+  if (!out) return fail(HSP_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!X || !y) return fail(HSP_EINVAL, "X or y is NULL");
+  if (x_dtype != HSP_F32 && x_dtype != HSP_F64) return fail(HSP_EINVAL, "x_dtype must be HSP_F32 or HSP_F64");
+  if (N < 2) return fail(HSP_EINVAL, "N must be >= 2");
+  if (p < 1) return fail(HSP_EINVAL, "p must be >= 1");
+  if (reinterpret_cast<uintptr_t>(X) % (x_dtype == HSP_F32 ? 4 : 8)) return fail(HSP_EINVAL, "X is misaligned");
+  cudaPointerAttributes pa{};
+  if (cudaPointerGetAttributes(&pa, X) != cudaSuccess || (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)) {
+    cudaGetLastError();
+    return fail(HSP_EINVAL, "X must be a device pointer");
+  }
+  if (cudaPointerGetAttributes(&pa, y) != cudaSuccess || (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)) {
+    cudaGetLastError();
+    return fail(HSP_EINVAL, "y must be a device pointer");
+  }
+  hsp_state* s = new (std::nothrow) hsp_state();
+  if (!s) return fail(HSP_ENOMEM, "out of host memory");
+  s->X = X; s->dtype = x_dtype; s->y = y; s->N = N; s->p = p; s->seed = seed; s->stream = (cudaStream_t)stream;
+  const int rc = create_common(out, s);
+  if (rc != HSP_OK) { free_state(s); *out = nullptr; }
+  return rc;
+}
+
+int hsp_create_host(hsp_state** out, const void* X_host, int x_dtype, const unsigned char* y_host, long long N, int p,
+                    unsigned long long seed, void* stream) {
+  if (!out) return fail(HSP_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!X_host || !y_host) return fail(HSP_EINVAL, "X or y is NULL");
+  if (x_dtype != HSP_F32 && x_dtype != HSP_F64) return fail(HSP_EINVAL, "x_dtype must be HSP_F32 or HSP_F64");
+  if (N < 2) return fail(HSP_EINVAL, "N must be >= 2");
+  if (p < 1) return fail(HSP_EINVAL, "p must be >= 1");
+  hsp_state* s = new (std::nothrow) hsp_state();
+  if (!s) return fail(HSP_ENOMEM, "out of host memory");
+  s->dtype = x_dtype; s->N = N; s->p = p; s->seed = seed; s->stream = (cudaStream_t)stream;
+  const size_t xb = (size_t)N * p * (x_dtype == HSP_F32 ? 4 : 8);
+  cudaError_t e = cudaMalloc(&s->own_X, xb);
+  if (e == cudaSuccess) e = cudaMalloc(&s->own_y, (size_t)N);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(s->own_X, X_host, xb, cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(s->own_y, y_host, (size_t)N, cudaMemcpyHostToDevice, s->stream);
+  if (e != cudaSuccess) { const int rc = cuda_fail(e, "upload of X, y"); free_state(s); return rc; }
+  s->X = s->own_X; s->y = s->own_y;
+  const int rc = create_common(out, s);
+  if (rc != HSP_OK) { free_state(s); *out = nullptr; }
+  return rc;
+}
+
+int hsp_destroy(hsp_state* s) {
+  if (!s) return HSP_OK;
+  cudaStreamSynchronize(s->stream);
+  if (s->stream2) cudaStreamSynchronize(s->stream2);
+  free_state(s);
+  return HSP_OK;
+}
+
+int hsp_set_flags(hsp_state* s, unsigned flags) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  const unsigned known = HSP_STORE_Z | HSP_FREEZE_SCALES | HSP_FREEZE_Z | HSP_FREEZE_BETA | HSP_NO_GRAPH | HSP_SERIAL;
+  if (flags & ~known) return fail(HSP_EINVAL, "unknown flag");
+  if ((flags & HSP_STORE_Z) && !s->z) {
+    CK(cudaMalloc(&s->z, (size_t)s->N * sizeof(double)));
+    CK(cudaMemsetAsync(s->z, 0, (size_t)s->N * sizeof(double), s->stream));
+  }
+  s->flags = flags;
+  return HSP_OK;
+}
+
+int hsp_sweep(hsp_state* s, long long n_iter) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  if (n_iter < 0) return fail(HSP_EINVAL, "n_iter must be >= 0");
+  const int p = s->p;
+  if (n_iter > s->h_cap) {
+    CK(cudaStreamSynchronize(s->stream));
+    if (s->h_beta) { cudaFree(s->h_beta); cudaFree(s->h_lambda); cudaFree(s->h_tau); s->h_beta = s->h_lambda = s->h_tau = nullptr; }
+    s->h_cap = 0;
+    CK(cudaMalloc(&s->h_beta, (size_t)n_iter * p * sizeof(double)));
+    CK(cudaMalloc(&s->h_lambda, (size_t)n_iter * p * sizeof(double)));
+    CK(cudaMalloc(&s->h_tau, (size_t)n_iter * sizeof(double)));
+    s->h_cap = n_iter;
+  }
+  s->h_n = n_iter;
+  if (n_iter == 0) return HSP_OK;
+  // history window of this call: only these fields of Ctl are touched from the host
+  struct { unsigned long long hist_base; } hb{(unsigned long long)s->host_sweep};
+  CK(cudaMemcpyAsync(reinterpret_cast<char*>(s->ctl) + offsetof(Ctl, hist_base), &hb, sizeof(hb), cudaMemcpyHostToDevice, s->stream));
+  double* hp[3] = {s->h_beta, s->h_lambda, s->h_tau};
+  CK(cudaMemcpyAsync(reinterpret_cast<char*>(s->ctl) + offsetof(Ctl, h_beta), hp, sizeof(hp), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaStreamSynchronize(s->stream));   // hb / hp are stack temporaries
+  if (s->flags & HSP_STORE_Z) s->z_valid = !(s->flags & HSP_FREEZE_Z) || s->z_valid;
+  else if (!(s->flags & HSP_FREEZE_Z)) s->z_valid = false;
+  if (s->flags & HSP_NO_GRAPH) {
+    for (long long it = 0; it < n_iter; ++it) {
+      if (s->tev_used >= 8192) { CK(cudaStreamSynchronize(s->stream)); const int rc = drain_fused_events(s); if (rc) return rc; }
+      long long k = 0;
+      const int rc = enqueue_sweep(s, true, &k);
+      if (rc != HSP_OK) return rc;
+      s->launches += k;
+    }
+  } else {
+    if (!s->graph_exec || s->graph_flags != s->flags) {
+      const int rc = build_graph(s);
+      if (rc != HSP_OK) return rc;
+    }
+    for (long long it = 0; it < n_iter; ++it) CK(cudaGraphLaunch(s->graph_exec, s->stream));
+    s->launches += s->graph_kernels * n_iter;
+  }
+  s->host_sweep += n_iter;
+  return HSP_OK;
+}
+
+static int sync_status(const hsp_state* s) {
+  CK(cudaStreamSynchronize(s->stream));
+  int st = 0;
+  CK(cudaMemcpy(&st, reinterpret_cast<const char*>(s->ctl) + offsetof(Ctl, status), sizeof(int), cudaMemcpyDeviceToHost));
+  if (st == HSP_ENOTPD) return fail(HSP_ENOTPD, "Cholesky breakdown: Q is not positive definite");
+  if (st == HSP_ENUMERIC) return fail(HSP_ENUMERIC, "non-finite value in the chain state");
+  return HSP_OK;
+}
+
+int hsp_sync(const hsp_state* s) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  return sync_status(s);
+}
+
+int hsp_get_draws(const hsp_state* s, double* beta, double* lambda, double* tau) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  const int rc = sync_status(s);
+  const size_t np = (size_t)s->h_n * s->p * sizeof(double);
+  if (s->h_n > 0) {
+    if (beta) CK(cudaMemcpy(beta, s->h_beta, np, cudaMemcpyDefault));
+    if (lambda) CK(cudaMemcpy(lambda, s->h_lambda, np, cudaMemcpyDefault));
+    if (tau) CK(cudaMemcpy(tau, s->h_tau, (size_t)s->h_n * sizeof(double), cudaMemcpyDefault));
+  }
+  return rc;
+}
+
+int hsp_get_latent(const hsp_state* s, double* z, signed char* side) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  CK(cudaStreamSynchronize(s->stream));
+  if (z) {
+    if (!s->z || !s->z_valid) return fail(HSP_EINVAL, "z was not stored: set HSP_STORE_Z before hsp_sweep");
+    CK(cudaMemcpy(z, s->z, (size_t)s->N * sizeof(double), cudaMemcpyDefault));
+  }
+  if (side) {
+    hsp_state* m = const_cast<hsp_state*>(s);
+    if (!m->side) CK(cudaMalloc(&m->side, (size_t)s->N));
+    CK(side_launch(s->y, s->N, m->side, s->stream));
+    m->launches += 1;
+    CK(cudaStreamSynchronize(s->stream));
+    CK(cudaMemcpy(side, m->side, (size_t)s->N, cudaMemcpyDefault));
+  }
+  return HSP_OK;
+}
+
+int hsp_get_state(const hsp_state* s, double* beta, double* lam_inv2, double* nu_inv, double* tau_inv2, double* xi_inv,
+                  long long* sweep) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  const int rc = sync_status(s);
+  const size_t pv = (size_t)s->p * sizeof(double);
+  if (beta) CK(cudaMemcpy(beta, s->beta, pv, cudaMemcpyDefault));
+  if (lam_inv2) CK(cudaMemcpy(lam_inv2, s->lam_inv2, pv, cudaMemcpyDefault));
+  if (nu_inv) CK(cudaMemcpy(nu_inv, s->nu_inv, pv, cudaMemcpyDefault));
+  Ctl c{};
+  CK(cudaMemcpy(&c, s->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost));
+  if (tau_inv2) CK(cudaMemcpy(tau_inv2, &c.tau_inv2, sizeof(double), cudaMemcpyDefault));
+  if (xi_inv) CK(cudaMemcpy(xi_inv, &c.xi_inv, sizeof(double), cudaMemcpyDefault));
+  if (sweep) *sweep = (long long)c.sweep;
+  return rc;
+}
+
+int hsp_set_state(hsp_state* s, const double* beta, const double* lam_inv2, const double* nu_inv, const double* tau_inv2,
+                  const double* xi_inv, long long sweep) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  CK(cudaStreamSynchronize(s->stream));
+  const size_t pv = (size_t)s->p * sizeof(double);
+  if (beta) CK(cudaMemcpy(s->beta, beta, pv, cudaMemcpyDefault));
+  if (lam_inv2) CK(cudaMemcpy(s->lam_inv2, lam_inv2, pv, cudaMemcpyDefault));
+  if (nu_inv) CK(cudaMemcpy(s->nu_inv, nu_inv, pv, cudaMemcpyDefault));
+  char* c = reinterpret_cast<char*>(s->ctl);
+  if (tau_inv2) CK(cudaMemcpy(c + offsetof(Ctl, tau_inv2), tau_inv2, sizeof(double), cudaMemcpyDefault));
+  if (xi_inv) CK(cudaMemcpy(c + offsetof(Ctl, xi_inv), xi_inv, sizeof(double), cudaMemcpyDefault));
+  if (sweep >= 0) {
+    const unsigned long long k = (unsigned long long)sweep;
+    CK(cudaMemcpy(c + offsetof(Ctl, sweep), &k, sizeof(k), cudaMemcpyHostToDevice));
+    s->host_sweep = sweep;
+  }
+  const int zero = 0;
+  CK(cudaMemcpy(c + offsetof(Ctl, status), &zero, sizeof(int), cudaMemcpyHostToDevice));
+  return HSP_OK;
+}
+
+int hsp_get_xtz(const hsp_state* s, double* g) {
+  if (!s || !g) return fail(HSP_EINVAL, "NULL argument");
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaMemcpy(g, s->g, (size_t)s->p * sizeof(double), cudaMemcpyDefault));
+  return HSP_OK;
+}
+int hsp_get_gram(const hsp_state* s, double* G) {
+  if (!s || !G) return fail(HSP_EINVAL, "NULL argument");
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaMemcpy(G, s->G, (size_t)s->p * s->p * sizeof(double), cudaMemcpyDefault));
+  return HSP_OK;
+}
+int hsp_get_chol(const hsp_state* s, double* L) {
+  if (!s || !L) return fail(HSP_EINVAL, "NULL argument");
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaMemcpy(L, s->L, (size_t)s->p * s->p * sizeof(double), cudaMemcpyDefault));
+  return HSP_OK;
+}
+
+int hsp_get_fused_pass_ms(hsp_state* s, double* ms, long long* launches) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  CK(cudaStreamSynchronize(s->stream));
+  const int rc = drain_fused_events(s);
+  if (rc != HSP_OK) return rc;
+  if (ms) *ms = s->fused_n ? s->fused_ms_sum / (double)s->fused_n : 0.0;
+  if (launches) *launches = s->fused_n;
+  s->fused_ms_sum = 0.0; s->fused_n = 0;
+  return HSP_OK;
+}
+
+long long hsp_get_launch_count(const hsp_state* s) { return s ? s->launches : 0; }
+const char* hsp_fused_variant(const hsp_state* s) { return (s && s->plan.variant == 1) ? "tma" : "generic"; }
+
+// ---- device unit-test hooks ----------------------------------------------------------------------
+__global__ void dbg_philox_kernel(const unsigned* ctr, const unsigned* key, unsigned* out, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  U4 c{ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3]};
+  const U4 r = philox4x32_10(c, key[2 * i], key[2 * i + 1]);
+  out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+}
+__global__ void dbg_uniform_kernel(unsigned long long seed, const unsigned long long* idx, unsigned sweep, unsigned tag,
+                                   double* ua, double* ub, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const U4 r = variate_bits(seed, idx[i], sweep, tag);
+  if (ua) ua[i] = bits_to_unit(r.x, r.y);
+  if (ub) ub[i] = bits_to_unit(r.z, r.w);
+}
+__global__ void dbg_tnpos_kernel(const double* m, const double* u, double* w, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool ok = i < n;
+  const double r = tnpos(ok ? m[i] : 0.0, ok ? u[i] : 0.5);   // all lanes call: the tail vote is warp-wide
+  if (ok) w[i] = r;
+}
+__global__ void dbg_norm_inv_kernel(const double* u, double* x, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) x[i] = norm_inv(u[i]);
+}
+__global__ void dbg_cheng_kernel(double alpha, unsigned long long seed, unsigned sweep0, double* x, long long n) {
+  const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (w >= n) return;   // warp-uniform
+  const double r = cheng_gamma_warp(alpha, seed, sweep0 + (unsigned)w);
+  if ((threadIdx.x & 31) == 0) x[w] = r;
+}
+
+int hsp_dbg_philox(const unsigned* ctr, const unsigned* key, unsigned* out, long long n, void* stream) {
+  if (n <= 0) return HSP_OK;
+  dbg_philox_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(ctr, key, out, n);
+  CK(cudaGetLastError());
+  return HSP_OK;
+}
+int hsp_dbg_uniform(unsigned long long seed, const unsigned long long* idx, unsigned sweep, unsigned tag, double* ua,
+                    double* ub, long long n, void* stream) {
+  if (n <= 0) return HSP_OK;
+  dbg_uniform_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(seed, idx, sweep, tag, ua, ub, n);
+  CK(cudaGetLastError());
+  return HSP_OK;
+}
+int hsp_dbg_tnpos(const double* m, const double* u, double* w, long long n, void* stream) {
+  if (n <= 0) return HSP_OK;
+  dbg_tnpos_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(m, u, w, n);
+  CK(cudaGetLastError());
+  return HSP_OK;
+}
+int hsp_dbg_norm_inv(const double* u, double* x, long long n, void* stream) {
+  if (n <= 0) return HSP_OK;
+  dbg_norm_inv_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(u, x, n);
+  CK(cudaGetLastError());
+  return HSP_OK;
+}
+int hsp_dbg_cheng(double alpha, unsigned long long seed, unsigned sweep0, double* x, long long n, void* stream) {
+  if (n <= 0) return HSP_OK;
+  dbg_cheng_kernel<<<(unsigned)((n * 32 + 255) / 256), 256, 0, (cudaStream_t)stream>>>(alpha, seed, sweep0, x, n);
+  CK(cudaGetLastError());
+  return HSP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,60 @@
+// hsp_internal.h -- host-side declarations shared by the translation units of libhsp.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace hsp {
+
+// Device-resident control block: everything a captured CUDA graph must read at replay time.
+struct Ctl {
+  unsigned long long sweep;      // number of completed sweeps k
+  unsigned long long hist_base;  // sweep count when the current hsp_sweep call started
+  double tau_inv2;               // tau^-2
+  double xi_inv;                 // xi^-1
+  int status;                    // 0, or HSP_ENOTPD / HSP_ENUMERIC (first error wins)
+  int pad;
+  double* h_beta;                // device history of the current hsp_sweep call (may be null)
+  double* h_lambda;
+  double* h_tau;
+};
+
+enum { kF32 = 0, kF64 = 1 };
+
+struct FusedPlan {
+  int variant;        // 0 = generic, 1 = tma
+  int grid, block;
+  size_t smem;
+  int rows_per_tile;  // R
+  int stages;         // S
+  int lag;            // D
+  int chunks;         // C
+  long long n_tiles;
+};
+
+// ---- fused pass (a1-a3) and reduce (b): fused_pass.cu
+FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X);
+cudaError_t fused_pass_launch(const FusedPlan& plan, const void* X, int dtype, const unsigned char* y, long long N,
+                              int p, unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
+                              double* z_out, cudaStream_t st);
+cudaError_t reduce_partials_launch(const double* partial, int n_part, int p, double* g, cudaStream_t st);
+
+// ---- Gram (c0): gram.cu
+cudaError_t gram_launch(const void* X, int dtype, long long N, int p, double* G, double* scratch, int splits,
+                        cudaStream_t st);
+int gram_splits(long long N, int p, int num_sms);
+
+// ---- Q build (c), Cholesky (d1), beta draw (d2): cholesky.cu
+cudaError_t build_q_launch(const double* G, const double* lam_inv2, const Ctl* ctl, double* L, int p, cudaStream_t st);
+cudaError_t cholesky_launch(double* L, int p, Ctl* ctl, cudaStream_t st, long long* launches);
+cudaError_t beta_draw_launch(const double* L, const double* g, double* beta, int p, unsigned long long seed,
+                             Ctl* ctl, cudaStream_t st);
+
+// ---- scale conditionals (e1, e2, e3) and draw output (g): scales.cu
+cudaError_t scales_pre_launch(const double* beta, double* lam_inv2, const double* nu_inv, Ctl* ctl, int p,
+                              unsigned long long seed, cudaStream_t st);
+cudaError_t scales_post_launch(const double* beta, const double* lam_inv2, double* nu_inv, Ctl* ctl, int p,
+                               unsigned long long seed, int freeze_scales, cudaStream_t st);
+cudaError_t validate_y_launch(const unsigned char* y, long long N, int* bad, cudaStream_t st);
+cudaError_t side_launch(const unsigned char* y, long long N, signed char* side, cudaStream_t st);
+
+}  // namespace hsp
