@@ -119,6 +119,11 @@ __device__ __forceinline__ int row_of_lane(int lane) {
   return row;
 }
 
+static int env_int(const char* name, int dflt) {
+  const char* v = getenv(name);
+  return (v && *v) ? atoi(v) : dflt;
+}
+
 constexpr int kComputeWarps = 8;
 constexpr int kComputeThreads = kComputeWarps * 32;
 constexpr int kSamplerWarps = 4;
@@ -141,7 +146,7 @@ template <typename XT, int RT, int C>
 __global__ void __launch_bounds__(kTmaThreads, 1)
 fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
                unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
-               double* __restrict__ partial, double* __restrict__ z_out, int S, int D, long long n_tiles) {
+               double* __restrict__ partial, double* __restrict__ z_out, int S, int D, long long n_tiles, int dbg) {
   constexpr int V = Vec<XT>::V;
   using Acc = typename Vec<XT>::Acc;
   constexpr bool kF32 = sizeof(XT) == 4;
@@ -172,14 +177,22 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // Zero the ring once: rows of a ragged last tile that TMA does not write are then finite
+  // (stale or zero) and contribute x * 0 = 0 in the xz phase, so the inner loops need no row guards.
+  {
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+    for (size_t o = (size_t)tid * 16; o < (size_t)S * stage_bytes; o += (size_t)kTmaThreads * 16)
+      *reinterpret_cast<uint4*>(tiles + o) = zero;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes before TMA writes
+  }
   __syncthreads();
 
   if (warp == kComputeWarps + kSamplerWarps) {
     // ===================== producer: one thread streams the tiles =====================
     if (lane == 0) {
+      int st = 0;
+      uint32_t ph = 0;
       for (long long n = 0; n < my_tiles; ++n) {
-        const int st = (int)(n % S);
-        const uint32_t ph = (uint32_t)((n / S) & 1);
         mbar_wait(&empty[st], ph ^ 1u);
         const long long row0 = (cta + n * grid) * RT;
         const long long rows = (N - row0) < RT ? (N - row0) : RT;
@@ -187,44 +200,64 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         mbar_arrive_expect_tx(&full[st], bytes);
         bulk_g2s(tiles + (size_t)st * stage_bytes, reinterpret_cast<const unsigned char*>(X) + (size_t)row0 * row_bytes,
                  bytes, &full[st]);
+        if (++st == S) { st = 0; ph ^= 1u; }
       }
     }
   } else if (warp >= kComputeWarps) {
     // ===================== sampler warps: eta -> z, D tiles behind the eta phase =====================
+    // Tile n goes to sampler warp n mod ns.  ns <= S keeps every mbarrier wait at most one phase
+    // behind (a waiter two phases behind would alias on the parity bit).
     const int sw = warp - kComputeWarps;
-    for (long long n = sw; n < my_tiles; n += kSamplerWarps) {
-      const int st = (int)(n % S);
-      const uint32_t ph = (uint32_t)((n / S) & 1);
-      const long long row0 = (cta + n * grid) * RT;
-      // everything that does not depend on eta first: y, the Philox uniform
-      const long long i = row0 + lane;
-      const bool valid = (lane < RT) && (i < N);
-      const double ystar = valid ? 2.0 * (double)y[i] - 1.0 : 1.0;
-      const double u = uniform_a(seed, (unsigned long long)(valid ? i : 0), sweep, TAG_Z);
-      mbar_wait(&eta_full[st], ph);
-      double eta = 0.0;
-      if (lane < RT) {
+    const int ns = S < kSamplerWarps ? S : kSamplerWarps;
+    if (sw < ns) {
+      // y is prefetched three tiles ahead: under a saturated HBM a lone 1-byte load takes microseconds
+      auto load_y = [&](long long n) -> int {
+        const long long i = (cta + n * grid) * RT + lane;
+        return (n < my_tiles && lane < RT && i < N) ? (int)y[i] : 1;
+      };
+      int y0 = load_y(sw), y1 = load_y(sw + ns), y2 = load_y(sw + 2LL * ns);
+      int st = sw;                  // sw < ns <= S
+      uint32_t ph = 0;
+      for (long long n = sw; n < my_tiles; n += ns) {
+        const long long i = (cta + n * grid) * RT + lane;
+        const bool valid = (lane < RT) && (i < N);
+        const int y3 = load_y(n + 3LL * ns);
+        // the Philox uniform does not depend on eta either: compute it before waiting
+        const double u = uniform_a(seed, (unsigned long long)(valid ? i : 0), sweep, TAG_Z);
+        const double ystar = 2.0 * (double)y0 - 1.0;
+        mbar_wait(&eta_full[st], ph);
+        double eta = 0.0;
+        if (lane < RT) {
+          const double* ep = eta_part + (size_t)st * kComputeWarps * RT + lane;
 #pragma unroll
-        for (int w = 0; w < kComputeWarps; ++w) eta += eta_part[((size_t)st * kComputeWarps + w) * RT + lane];
+          for (int w = 0; w < kComputeWarps; ++w) eta += ep[w * RT];
+        }
+        const double wpos = (dbg & 1) ? fabs(eta) + u : tnpos(ystar * eta, u);
+        const double z = valid ? ystar * wpos : 0.0;
+        if (lane < RT) {
+          z64[st * RT + lane] = z;
+          z32[st * RT + lane] = (float)z;
+        }
+        if (valid && z_out != nullptr) z_out[i] = z;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&z_full[st]);
+        y0 = y1; y1 = y2; y2 = y3;
+        st += ns;
+        if (st >= S) { st -= S; ph ^= 1u; }
       }
-      const double wpos = tnpos(ystar * eta, u);
-      const double z = valid ? ystar * wpos : 0.0;
-      if (lane < RT) {
-        z64[st * RT + lane] = z;
-        z32[st * RT + lane] = (float)z;
-      }
-      if (valid && z_out != nullptr) z_out[i] = z;
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&z_full[st]);
     }
   } else {
     // ===================== compute warps: eta partials, then x*z from the same stage =====================
+    // Thread t owns the 16-byte column stripes (c*256 + t)*V.  Stripes past p read column 0 with
+    // beta = 0 and are never written back, so the loops below are straight-line code.
     double breg[C][V];
     double acc64[C][V];
     Acc acc[C][V];
+    uint32_t coff[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) {
       const int col = (c * kComputeThreads + tid) * V;
+      coff[c] = (col < p) ? (uint32_t)(col * sizeof(XT)) : 0u;
 #pragma unroll
       for (int v = 0; v < V; ++v) {
         breg[c][v] = (col + v < p) ? beta[col + v] : 0.0;
@@ -234,59 +267,77 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     }
     const int my_row = row_of_lane<RT>(lane);
     const bool writer = (lane & (32 / RT - 1)) == 0;
+    const uint32_t rb = (uint32_t)row_bytes;
     int rows_since_flush = 0;
-    for (long long it = 0; it < my_tiles + D; ++it) {
-      if (it < my_tiles) {
-        const int st = (int)(it % S);
-        const uint32_t ph = (uint32_t)((it / S) & 1);
-        mbar_wait(&full[st], ph);
-        const unsigned char* tile = tiles + (size_t)st * stage_bytes;
+    int st_e = 0, st_g = 0;
+    uint32_t ph_e = 0, ph_g = 0;
+    const int total_it = (int)my_tiles + D;
+    for (int it = 0; it < total_it; ++it) {
+      if (it < (int)my_tiles) {
+        mbar_wait(&full[st_e], ph_e);
+        const unsigned char* tile = tiles + (size_t)st_e * stage_bytes;
         double part[RT];
 #pragma unroll
         for (int r = 0; r < RT; ++r) part[r] = 0.0;
+        if (!(dbg & 2)) {
 #pragma unroll
-        for (int c = 0; c < C; ++c) {
-          const int col = (c * kComputeThreads + tid) * V;
-          if (col < p) {
+          for (int c = 0; c < C; ++c) {
+            Vec<XT> x[RT];
 #pragma unroll
-            for (int r = 0; r < RT; ++r) {
-              Vec<XT> x;
-              x.load(tile + (size_t)r * row_bytes + (size_t)col * sizeof(XT));
-              part[r] += x.dot(breg[c]);
-            }
+            for (int r = 0; r < RT; ++r) x[r].load(tile + r * rb + coff[c]);
+#pragma unroll
+            for (int r = 0; r < RT; ++r) part[r] += x[r].dot(breg[c]);
           }
         }
         const double tot = warp_reduce_rows<RT>(part, lane);
-        if (writer) eta_part[((size_t)st * kComputeWarps + warp) * RT + my_row] = tot;
+        if (writer) eta_part[((size_t)st_e * kComputeWarps + warp) * RT + my_row] = tot;
         __syncwarp();
-        if (lane == 0) mbar_arrive(&eta_full[st]);
+        if (lane == 0) mbar_arrive(&eta_full[st_e]);
+        if (++st_e == S) { st_e = 0; ph_e ^= 1u; }
       }
       if (it >= D) {
-        const long long n2 = it - D;
-        const int st = (int)(n2 % S);
-        const uint32_t ph = (uint32_t)((n2 / S) & 1);
-        mbar_wait(&z_full[st], ph);
-        const unsigned char* tile = tiles + (size_t)st * stage_bytes;
-        const long long row0 = (cta + n2 * grid) * RT;
-        const int nrows = (N - row0) < RT ? (int)(N - row0) : RT;
+        mbar_wait(&z_full[st_g], ph_g);
+        const unsigned char* tile = tiles + (size_t)st_g * stage_bytes;
+        Acc zr[RT];
+        if constexpr (kF32) {
+          const float* zp = z32 + st_g * RT;
+          if constexpr (RT % 4 == 0) {
 #pragma unroll
-        for (int r = 0; r < RT; ++r) {
-          if (r < nrows) {
-            Acc zr;
-            if constexpr (kF32) zr = z32[st * RT + r]; else zr = z64[st * RT + r];
-#pragma unroll
-            for (int c = 0; c < C; ++c) {
-              const int col = (c * kComputeThreads + tid) * V;
-              if (col < p) {
-                Vec<XT> x;
-                x.load(tile + (size_t)r * row_bytes + (size_t)col * sizeof(XT));
-                x.axpy(zr, acc[c]);
-              }
+            for (int q = 0; q < RT / 4; ++q) {
+              const float4 t = *reinterpret_cast<const float4*>(zp + 4 * q);
+              zr[4 * q] = t.x; zr[4 * q + 1] = t.y; zr[4 * q + 2] = t.z; zr[4 * q + 3] = t.w;
             }
+          } else if constexpr (RT == 2) {
+            const float2 t = *reinterpret_cast<const float2*>(zp);
+            zr[0] = t.x; zr[1] = t.y;
+          } else {
+            zr[0] = zp[0];
+          }
+        } else {
+          const double* zp = z64 + st_g * RT;
+          if constexpr (RT % 2 == 0) {
+#pragma unroll
+            for (int q = 0; q < RT / 2; ++q) {
+              const double2 t = *reinterpret_cast<const double2*>(zp + 2 * q);
+              zr[2 * q] = t.x; zr[2 * q + 1] = t.y;
+            }
+          } else {
+            zr[0] = zp[0];
+          }
+        }
+        if (!(dbg & 4)) {
+#pragma unroll
+          for (int c = 0; c < C; ++c) {
+            Vec<XT> x[RT];
+#pragma unroll
+            for (int r = 0; r < RT; ++r) x[r].load(tile + r * rb + coff[c]);
+#pragma unroll
+            for (int r = 0; r < RT; ++r) x[r].axpy(zr[r], acc[c]);
           }
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[st]);
+        if (lane == 0) mbar_arrive(&empty[st_g]);
+        if (++st_g == S) { st_g = 0; ph_g ^= 1u; }
         if constexpr (kF32) {
           rows_since_flush += RT;
           if (rows_since_flush >= kFlushRows) {
@@ -401,10 +452,6 @@ __global__ void reduce_partials_kernel(const double* __restrict__ partial, int n
 // ------------------------------------------------------------------------------------------------
 // Host side: variant selection and launch
 // ------------------------------------------------------------------------------------------------
-static int env_int(const char* name, int dflt) {
-  const char* v = getenv(name);
-  return (v && *v) ? atoi(v) : dflt;
-}
 
 static int round_chunks(int c) {
   const int opts[] = {1, 2, 3, 4, 6, 8, 12, 16};
@@ -469,7 +516,7 @@ static cudaError_t launch_tma(const FusedPlan& pl, const void* X, const unsigned
   }
   if (N < 0) return cudaSuccess;     // prepare-only call (sets the attribute outside stream capture)
   kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
-                                          pl.stages, pl.lag, pl.n_tiles);
+                                          pl.stages, pl.lag, pl.n_tiles, env_int("HSP_FUSED_DEBUG", 0));
   return cudaGetLastError();
 }
 
