@@ -1,247 +1,439 @@
 // cholesky.cu -- rows c, d1, d2 of the hot-path table:
 //   c   Q = G + diag(tau^-2 lam_j^-2)
-//   d1  Q = L L^T, blocked right-looking fp64 Cholesky
-//   d2  beta = Q^-1 g + L^-T e  via  L v = g,  L^T beta = v + e,  e_j = Phi^-1(u_j)
-//                                                            PAPER.md:180, 198-202, 239 (reading R5)
-// Storage: row-major p x p, lower triangle.
+//   d1  Q = L L^T, tiled fp64 Cholesky
+//   d2  beta = Q^-1 g + L^-T e,  e_j = Phi^-1(u_j)           PAPER.md:180, 198-202, 239 (reading R5)
+//
+// One persistent kernel (`chol_dataflow_kernel`) does c and d1 and, in the same task graph, the inverse
+// factor W = L^-1 (and its transpose Wt = L^-T): d2 then needs no substitution on the critical path
+// after X^T z arrives -- it is two triangular matrix-vector products, t = W g + e and beta = Wt t,
+// i.e. L t = g + L e and L^T beta = t, exactly the two solves of PAPER.md:199-201.
+//
+// Task graph on 64x64 tiles (nt = ceil(p/64) tile rows; matrices padded to P = 64 nt with the identity):
+//   L(i,j), i >= j :  A = Q_ij - sum_{k<j} L_ik L_jk^T ;  i == j: L_jj = chol(A), W_jj = L_jj^-1 ;
+//                                                         i >  j: L_ij = A W_jj^T
+//   B(i,j), i <  j :  A = - sum_{k=i}^{j-1} L_jk Wt_ik^T ; W_ji = W_jj A  (stored in W and, transposed, in Wt)
+// Tasks are numbered column by column and dealt round-robin to the CTAs; every task depends only on
+// lower-numbered tasks, each CTA runs its tasks in order, and all CTAs are co-resident (cooperative
+// launch), so spinning on the per-tile "done" flags cannot deadlock.  Every tile is computed by one
+// CTA with a fixed summation order: the result does not depend on the number of CTAs.
+//
+// Storage: row-major, leading dimension P; L lower, W lower, Wt upper.
 #include <cuda_runtime.h>
 #include <cstdint>
+#include <cstdlib>
 #include "hsp_device.cuh"
 #include "hsp_internal.h"
 
 namespace hsp {
 
-constexpr int NB = 32;   // panel width
+constexpr int CT = 64;                 // tile edge
+constexpr int KC = 16;                 // k-columns per pipeline chunk
+constexpr int CLD = KC + 2;            // chunk row stride in doubles (144 B): conflict-free LDS.128
+constexpr int TLD = CT + 2;            // full-tile row stride in shared memory (528 B)
+constexpr int NST = 4;                 // cp.async pipeline stages
+constexpr int kCholThreads = 256;
+constexpr int kStageDoubles = 2 * CT * CLD;                       // A chunk + B chunk
+constexpr size_t kCholSmem = (size_t)NST * kStageDoubles * sizeof(double) + 1024;   // 73728 + scratch
+static_assert((size_t)NST * kStageDoubles >= 2 * (size_t)CT * TLD, "finalize tiles must fit in the pipeline pool");
 
-__global__ void build_q_kernel(const double* __restrict__ G, const double* __restrict__ lam_inv2,
-                               const Ctl* __restrict__ ctl, double* __restrict__ L, int p) {
-  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= (size_t)p * p) return;
-  const int i = (int)(idx / p), j = (int)(idx % p);
-  if (j > i) return;
-  double v = G[idx];
-  if (i == j) v += ctl->tau_inv2 * lam_inv2[j];
-  L[idx] = v;
+int chol_tiles(int p) { return (p + CT - 1) / CT; }
+int chol_ld(int p) { return chol_tiles(p) * CT; }
+size_t chol_flag_count(int p) { const size_t nt = chol_tiles(p); return 2 * nt * nt; }
+
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ int ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void wait_flag(const int* f) {
+  while (ld_acquire(f) == 0) __nanosleep(32);
 }
 
-// Panel step at column k0: every CTA factors the NB x NB diagonal block (warp 0, rows in
-// registers, shuffles) redundantly, CTA 0 writes it back, and each CTA then solves its 128 rows of
-// the block column below:  L21 = A21 L11^-T  (thread per row, forward substitution).
-constexpr int kPanelRows = 128;
-__global__ void __launch_bounds__(kPanelRows)
-chol_panel_kernel(double* __restrict__ A, int p, int k0, Ctl* __restrict__ ctl) {
-  __shared__ double D[NB][NB + 1];
-  __shared__ double invd[NB];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int nb = (p - k0) < NB ? (p - k0) : NB;
-  if (warp == 0) {
-    double a[NB];
-    const int i = lane;
+// acc[a][b] (rows ty+16a, cols tx+16b) += sgn * sum_k A[row][k] B[col][k],  k in [0, K), K even.
+template <int LDA, int LDB, int K, bool NEG>
+__device__ __forceinline__ void tile_mac(const double* __restrict__ A, const double* __restrict__ B, int ty, int tx,
+                                         double (&acc)[4][4]) {
 #pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      double v = (i == j) ? 1.0 : 0.0;                       // identity padding past nb
-      if (i < nb && j <= i) v = A[(size_t)(k0 + i) * p + k0 + j];
-      a[j] = v;
-    }
-    bool bad = false;
+  for (int kk = 0; kk < K; kk += 2) {
+    double2 av[4], bv[4];
 #pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      double d = __shfl_sync(0xffffffffu, a[j], j);
-      if (!(d > 0.0)) { bad = true; d = 1.0; }
-      const double inv = rsqrt(d);
-      const double l = d * inv;
-      a[j] = (i == j) ? l : a[j] * inv;
+    for (int a = 0; a < 4; ++a) av[a] = *reinterpret_cast<const double2*>(A + (ty + 16 * a) * LDA + kk);
 #pragma unroll
-      for (int k = j + 1; k < NB; ++k) {
-        const double lkj = __shfl_sync(0xffffffffu, a[j], k);
-        a[k] = fma(-a[j], lkj, a[k]);
+    for (int b = 0; b < 4; ++b) bv[b] = *reinterpret_cast<const double2*>(B + (tx + 16 * b) * LDB + kk);
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        if (NEG) {
+          acc[a][b] = fma(-av[a].x, bv[b].x, acc[a][b]);
+          acc[a][b] = fma(-av[a].y, bv[b].y, acc[a][b]);
+        } else {
+          acc[a][b] = fma(av[a].x, bv[b].x, acc[a][b]);
+          acc[a][b] = fma(av[a].y, bv[b].y, acc[a][b]);
+        }
       }
-      if (i == j) invd[j] = 1.0 / l;
-    }
-    if (bad && lane == 0 && blockIdx.x == 0) atomicCAS(&ctl->status, 0, -4);
-#pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      D[i][j] = (j <= i) ? a[j] : 0.0;
-      if (blockIdx.x == 0 && i < nb && j <= i) A[(size_t)(k0 + i) * p + k0 + j] = a[j];
-    }
-  }
-  __syncthreads();
-  const int r = k0 + nb + blockIdx.x * kPanelRows + tid;
-  if (r < p) {
-    double a[NB];
-    double* row = A + (size_t)r * p + k0;
-#pragma unroll
-    for (int j = 0; j < NB; ++j) a[j] = (j < nb) ? row[j] : 0.0;
-#pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      double s = a[j];
-#pragma unroll
-      for (int k = 0; k < j; ++k) s = fma(-a[k], D[j][k], s);
-      a[j] = s * invd[j];
-    }
-#pragma unroll
-    for (int j = 0; j < NB; ++j)
-      if (j < nb) row[j] = a[j];
   }
 }
 
-// Trailing update after panel k0:  A22 -= L21 L21^T on lower 64x64 tiles (K = NB).
-constexpr int kUT = 64;
-__global__ void __launch_bounds__(256)
-chol_update_kernel(double* __restrict__ A, int p, int k0) {
-  __shared__ double As[NB][kUT + 4];
-  __shared__ double Bs[NB][kUT + 4];
-  int t = blockIdx.x, ti = 0;
-  while (t >= ti + 1) { t -= ti + 1; ++ti; }
-  const int tj = t;
-  const int base = k0 + NB;
-  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-  // load L21 rows of tile ti and tj: 64 rows x NB columns each, transposed into [k][row]
-  for (int e = tid; e < kUT * NB; e += 256) {
-    const int rr = e / NB, kk = e % NB;
-    const int ra = base + ti * kUT + rr, rb = base + tj * kUT + rr;
-    As[kk][rr] = (ra < p) ? A[(size_t)ra * p + k0 + kk] : 0.0;
-    Bs[kk][rr] = (rb < p) ? A[(size_t)rb * p + k0 + kk] : 0.0;
-  }
-  __syncthreads();
-  double acc[4][4];
+// In-place Cholesky of the 64x64 tile S (stride TLD, lower triangle used), all 256 threads.  On return
+// S holds L (lower, diagonal included; the strict upper triangle is zeroed).  One barrier per pivot:
+// the trailing update uses the unscaled column, S[r][c] -= S[r][j] S[c][j] / d_j, and the columns are
+// scaled by 1/sqrt(d_j) at the end.  Returns false if a pivot is not positive (then d_j := 1).
+__device__ __forceinline__ bool tile_potrf(double* __restrict__ S, double* __restrict__ dsq, int tid, int ty, int tx) {
+  bool ok = true;
+  for (int j = 0; j < CT; ++j) {
+    __syncthreads();
+    double d = S[j * TLD + j];
+    if (!(d > 0.0)) { ok = false; d = 1.0; }
+    const double inv = 1.0 / d;
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+    for (int a = 0; a < 4; ++a) {
+      const int r = ty + 16 * a;
+      if (r > j) {
+        const double lr = S[r * TLD + j] * inv;
 #pragma unroll
-    for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
-#pragma unroll
-  for (int kk = 0; kk < NB; ++kk) {
-    double a[4], b[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) { a[i] = As[kk][ty * 4 + i]; b[i] = Bs[kk][tx * 4 + i]; }
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-      for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
-  }
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int r = base + ti * kUT + ty * 4 + i;
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const int c = base + tj * kUT + tx * 4 + j;
-      if (r < p && c <= r) A[(size_t)r * p + c] -= acc[i][j];
-    }
-  }
-}
-
-cudaError_t build_q_launch(const double* G, const double* lam_inv2, const Ctl* ctl, double* L, int p, cudaStream_t st) {
-  const size_t n = (size_t)p * p;
-  build_q_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, lam_inv2, ctl, L, p);
-  return cudaGetLastError();
-}
-
-cudaError_t cholesky_launch(double* L, int p, Ctl* ctl, cudaStream_t st, long long* launches) {
-  for (int k0 = 0; k0 < p; k0 += NB) {
-    const int below = p - k0 - NB;
-    const int grid = below > 0 ? (below + kPanelRows - 1) / kPanelRows : 1;
-    chol_panel_kernel<<<grid, kPanelRows, 0, st>>>(L, p, k0, ctl);
-    if (launches) ++*launches;
-    if (below > 0) {
-      const int ts = (below + kUT - 1) / kUT;
-      chol_update_kernel<<<ts * (ts + 1) / 2, 256, 0, st>>>(L, p, k0);
-      if (launches) ++*launches;
-    }
-  }
-  return cudaGetLastError();
-}
-
-// d2: single-CTA blocked substitutions.  v = L^-1 g; beta = L^-T (v + e).
-constexpr int kSolveThreads = 512;
-__global__ void __launch_bounds__(kSolveThreads)
-beta_draw_kernel(const double* __restrict__ L, const double* __restrict__ g, double* __restrict__ beta, int p,
-                 unsigned long long seed, Ctl* __restrict__ ctl) {
-  extern __shared__ double v[];               // p doubles
-  __shared__ double xb[NB];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
-  for (int j = tid; j < p; j += kSolveThreads) v[j] = g[j];
-  __syncthreads();
-  // forward: L v = g
-  for (int k0 = 0; k0 < p; k0 += NB) {
-    const int nb = (p - k0) < NB ? (p - k0) : NB;
-    if (warp == 0) {
-      const int i = lane;
-      double a[NB];
-#pragma unroll
-      for (int j = 0; j < NB; ++j) a[j] = (i < nb && j < i) ? L[(size_t)(k0 + i) * p + k0 + j] : 0.0;
-      const double dinv = (i < nb) ? 1.0 / L[(size_t)(k0 + i) * p + k0 + i] : 1.0;
-      double r = (i < nb) ? v[k0 + i] : 0.0;
-#pragma unroll
-      for (int j = 0; j < NB; ++j) {
-        const double xj = __shfl_sync(0xffffffffu, r * dinv, j);
-        if (i == j) r = xj; else if (i > j) r = fma(-a[j], xj, r);
+        for (int b = 0; b < 4; ++b) {
+          const int c = tx + 16 * b;
+          if (c > j && c <= r) S[r * TLD + c] = fma(-lr, S[c * TLD + j], S[r * TLD + c]);
+        }
       }
-      if (i < nb) { v[k0 + i] = r; }
-      xb[i] = (i < nb) ? r : 0.0;
     }
-    __syncthreads();
-    for (int r = k0 + nb + tid; r < p; r += kSolveThreads) {
-      const double* row = L + (size_t)r * p + k0;
-      double s = v[r];
-#pragma unroll 8
-      for (int j = 0; j < nb; ++j) s = fma(-row[j], xb[j], s);
-      v[r] = s;
-    }
-    __syncthreads();
   }
-  // add e ~ N(0, I): one Philox call per coordinate
-  for (int j = tid; j < p; j += kSolveThreads) v[j] += norm_inv(uniform_a(seed, (unsigned long long)j, sweep, TAG_E));
   __syncthreads();
-  // backward: L^T beta = v
-  const int nblk = (p + NB - 1) / NB;
-  for (int b = nblk - 1; b >= 0; --b) {
-    const int k0 = b * NB;
-    const int nb = (p - k0) < NB ? (p - k0) : NB;
-    if (warp == 0) {
-      const int i = lane;                     // unknown k0 + i; needs column i of the diagonal block
-      double a[NB];
-#pragma unroll
-      for (int j = 0; j < NB; ++j) a[j] = (j < nb && i < nb && j > i) ? L[(size_t)(k0 + j) * p + k0 + i] : 0.0;
-      const double dinv = (i < nb) ? 1.0 / L[(size_t)(k0 + i) * p + k0 + i] : 1.0;
-      double r = (i < nb) ? v[k0 + i] : 0.0;
-#pragma unroll
-      for (int j = NB - 1; j >= 0; --j) {
-        const double xj = __shfl_sync(0xffffffffu, r * dinv, j);
-        if (i == j) r = xj; else if (i < j) r = fma(-a[j], xj, r);
-      }
-      if (i < nb) v[k0 + i] = r;
-      xb[i] = (i < nb) ? r : 0.0;
-    }
-    __syncthreads();
-    for (int r = tid; r < k0; r += kSolveThreads) {
-      double s = v[r];
-#pragma unroll 8
-      for (int j = 0; j < nb; ++j) s = fma(-L[(size_t)(k0 + j) * p + r], xb[j], s);
-      v[r] = s;
-    }
-    __syncthreads();
+  if (tid < CT) {
+    double d = S[tid * TLD + tid];
+    if (!(d > 0.0)) d = 1.0;
+    dsq[tid] = 1.0 / sqrt(d);
   }
-  bool bad = false;
-  for (int j = tid; j < p; j += kSolveThreads) {
-    const double b = v[j];
-    beta[j] = b;
-    if (!isfinite(b)) bad = true;
-  }
-  if (bad) atomicCAS(&ctl->status, 0, -5);
+  __syncthreads();
+  double v[4][4];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const int r = ty + 16 * a, c = tx + 16 * b;
+      double x = 0.0;
+      if (r > c) x = S[r * TLD + c] * dsq[c];
+      else if (r == c) { double d = S[r * TLD + r]; if (!(d > 0.0)) d = 1.0; x = d * dsq[r]; }
+      v[a][b] = x;
+    }
+  __syncthreads();
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) S[(ty + 16 * a) * TLD + tx + 16 * b] = v[a][b];
+  __syncthreads();
+  return ok;
 }
 
-cudaError_t beta_draw_launch(const double* L, const double* g, double* beta, int p, unsigned long long seed,
-                             Ctl* ctl, cudaStream_t st) {
-  const size_t smem = (size_t)p * sizeof(double);
-  static size_t configured = 0;
-  if (smem > 48 * 1024 && smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(beta_draw_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = smem;
+// X = S^-1 for the lower-triangular 64x64 tile S (stride TLD); X (stride TLD) gets the full tile
+// (zeros above the diagonal).  16x16 diagonal blocks by substitution (one thread per column, registers),
+// then two merge levels  [A 0; B C]^-1 = [A^-1 0; -C^-1 B A^-1  C^-1].
+__device__ __forceinline__ void tile_trinv(const double* __restrict__ S, const double* __restrict__ dsq,
+                                           double* __restrict__ X, int tid) {
+  for (int e = tid; e < CT * TLD; e += kCholThreads) X[e] = 0.0;
+  __syncthreads();
+  if (tid < CT) {
+    const int b0 = (tid >> 4) * 16, c = tid & 15;
+    double x[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+      double s = (r == c) ? 1.0 : 0.0;
+#pragma unroll
+      for (int m = 0; m < r; ++m) s = fma(-S[(b0 + r) * TLD + b0 + m], x[m], s);
+      x[r] = (r >= c) ? s * dsq[b0 + r] : 0.0;          // 1 / L_rr = 1 / sqrt(d_r)
+    }
+#pragma unroll
+    for (int r = 0; r < 16; ++r) X[(b0 + r) * TLD + b0 + c] = x[r];
   }
-  if (L == nullptr) return cudaSuccess;   // prepare-only call
-  beta_draw_kernel<<<1, kSolveThreads, smem, st>>>(L, g, beta, p, seed, ctl);
+  __syncthreads();
+  for (int h = 16; h < CT; h <<= 1) {
+    const int nblk = CT / (2 * h);
+    // T = B A^-1 into the (zero) upper-right block of X
+    for (int e = tid; e < nblk * h * h; e += kCholThreads) {
+      const int blk = e / (h * h), r = (e / h) % h, c = e % h, off = blk * 2 * h;
+      double s = 0.0;
+      for (int m = c; m < h; ++m) s = fma(S[(off + h + r) * TLD + off + m], X[(off + m) * TLD + off + c], s);
+      X[(off + r) * TLD + off + h + c] = s;
+    }
+    __syncthreads();
+    // lower-left block = -C^-1 T
+    for (int e = tid; e < nblk * h * h; e += kCholThreads) {
+      const int blk = e / (h * h), r = (e / h) % h, c = e % h, off = blk * 2 * h;
+      double s = 0.0;
+      for (int m = 0; m <= r; ++m) s = fma(X[(off + h + r) * TLD + off + h + m], X[(off + m) * TLD + off + h + c], s);
+      X[(off + h + r) * TLD + off + c] = -s;
+    }
+    __syncthreads();
+    for (int e = tid; e < nblk * h * h; e += kCholThreads) {
+      const int blk = e / (h * h), r = (e / h) % h, c = e % h, off = blk * 2 * h;
+      X[(off + r) * TLD + off + h + c] = 0.0;
+    }
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(kCholThreads, 1)
+chol_dataflow_kernel(const double* __restrict__ G, const double* __restrict__ lam_inv2, Ctl* __restrict__ ctl,
+                     double* __restrict__ L, double* __restrict__ W, double* __restrict__ Wt, int* __restrict__ flags,
+                     int p, int nt) {
+  extern __shared__ __align__(16) double pool[];
+  double* dsq = pool + (size_t)NST * kStageDoubles;          // 64 doubles of scratch after the pool
+  const int P = nt * CT;
+  const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+  int* fL = flags;
+  int* fB = flags + (size_t)nt * nt;
+  const double tau_inv2 = ctl->tau_inv2;
+  const long long ntasks = (long long)nt * nt;
+
+  for (long long t = blockIdx.x; t < ntasks; t += gridDim.x) {
+    const int j = (int)(t / nt), rr = (int)(t % nt);
+    const bool isL = rr < nt - j;
+    const int i = isL ? j + rr : rr - (nt - j);
+    // operands of the k loop: acc -= MA(ra,k) MB(rb,k)^T, k in [kbeg, kend)
+    const double* MA = L;
+    const double* MB = isL ? L : Wt;
+    const int ra = isL ? i : j, rb = isL ? j : i;
+    const int kbeg = isL ? 0 : i, kend = j;
+
+    double acc[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        double v = 0.0;
+        if (isL) {                                   // c: Q tile, padded with the identity
+          const int gr = i * CT + ty + 16 * a, gc = j * CT + tx + 16 * b;
+          if (gr < p && gc < p) {
+            v = G[(size_t)gr * p + gc];
+            if (gr == gc) v = fma(tau_inv2, lam_inv2[gr], v);
+          } else if (gr == gc) v = 1.0;
+        }
+        acc[a][b] = v;
+      }
+
+    const int nchunks = (kend - kbeg) * (CT / KC);
+    auto issue = [&](int c) {
+      const int k = kbeg + c / (CT / KC), kc = c % (CT / KC);
+      if (kc == 0) {                                 // first chunk of a k tile: its producers must be done
+        wait_flag(&fL[(size_t)ra * nt + k]);
+        if (isL) { if (rb != ra) wait_flag(&fL[(size_t)rb * nt + k]); }
+        else wait_flag(k == rb ? &fL[(size_t)rb * nt + rb] : &fB[(size_t)rb * nt + k]);
+      }
+      double* sa = pool + (size_t)(c % NST) * kStageDoubles;
+      double* sb = sa + CT * CLD;
+      const double* ga = MA + (size_t)ra * CT * P + (size_t)k * CT + kc * KC;
+      const double* gb = MB + (size_t)rb * CT * P + (size_t)k * CT + kc * KC;
+#pragma unroll
+      for (int q = tid; q < CT * (KC / 2); q += kCholThreads) {
+        const int row = q / (KC / 2), pc = q % (KC / 2);
+        cp_async16(sa + row * CLD + pc * 2, ga + (size_t)row * P + pc * 2);
+        cp_async16(sb + row * CLD + pc * 2, gb + (size_t)row * P + pc * 2);
+      }
+    };
+    __syncthreads();                                 // the pool is free (previous task's finalize is over)
+    for (int c = 0; c < NST - 1; ++c) {
+      if (c < nchunks) issue(c);
+      cp_async_commit();
+    }
+    for (int c = 0; c < nchunks; ++c) {
+      cp_async_wait<NST - 2>();
+      __syncthreads();
+      if (c + NST - 1 < nchunks) issue(c + NST - 1);
+      cp_async_commit();
+      const double* sa = pool + (size_t)(c % NST) * kStageDoubles;
+      tile_mac<CLD, CLD, KC, true>(sa, sa + CT * CLD, ty, tx, acc);
+    }
+    cp_async_wait<0>();
+    __syncthreads();
+
+    double* S = pool;                                // 64 x TLD
+    double* X = pool + CT * TLD;                     // 64 x TLD
+    if (isL && i == j) {
+      // ---- diagonal: L_jj = chol(acc), W_jj = L_jj^-1
+#pragma unroll
+      for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) S[(ty + 16 * a) * TLD + tx + 16 * b] = acc[a][b];
+      const bool ok = tile_potrf(S, dsq, tid, ty, tx);
+      if (!ok && tid == 0) atomicCAS(&ctl->status, 0, -4);
+      tile_trinv(S, dsq, X, tid);
+      for (int e = tid; e < CT * CT; e += kCholThreads) {
+        const int r = e / CT, c = e % CT;
+        const size_t g = (size_t)(j * CT + r) * P + j * CT + c;
+        L[g] = S[r * TLD + c];
+        W[g] = X[r * TLD + c];
+        Wt[g] = X[c * TLD + r];
+      }
+      __threadfence();
+      __syncthreads();
+      if (tid == 0) st_release(&fL[(size_t)j * nt + j], 1);
+    } else {
+      // ---- off-diagonal: multiply by W_jj (from global; written by the diagonal task of column j)
+      wait_flag(&fL[(size_t)j * nt + j]);
+      const double* wjj = W + (size_t)j * CT * P + (size_t)j * CT;
+      for (int q = tid; q < CT * (CT / 2); q += kCholThreads) {
+        const int row = q / (CT / 2), pc = q % (CT / 2);
+        cp_async16(X + row * TLD + pc * 2, wjj + (size_t)row * P + pc * 2);
+      }
+      cp_async_commit();
+      double out[4][4];
+#pragma unroll
+      for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) out[a][b] = 0.0;
+      if (isL) {
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) S[(ty + 16 * a) * TLD + tx + 16 * b] = acc[a][b];
+        cp_async_wait<0>();
+        __syncthreads();
+        tile_mac<TLD, TLD, CT, false>(S, X, ty, tx, out);          // L_ij = A W_jj^T
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) L[(size_t)(i * CT + ty + 16 * a) * P + j * CT + tx + 16 * b] = out[a][b];
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) st_release(&fL[(size_t)i * nt + j], 1);
+      } else {
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) S[(tx + 16 * b) * TLD + ty + 16 * a] = acc[a][b];   // transposed
+        cp_async_wait<0>();
+        __syncthreads();
+        tile_mac<TLD, TLD, CT, false>(X, S, ty, tx, out);          // W_ji = W_jj A
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) {
+            const int r = j * CT + ty + 16 * a, c = i * CT + tx + 16 * b;
+            W[(size_t)r * P + c] = out[a][b];
+            Wt[(size_t)c * P + r] = out[a][b];
+          }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) st_release(&fB[(size_t)i * nt + j], 1);
+      }
+    }
+  }
+}
+
+// d2, first half: t = W g + e (L t = g + L e), one warp per row; e_j = Phi^-1(U_A(j, k, E)).
+constexpr int kGemvWarps = 8;
+__global__ void __launch_bounds__(kGemvWarps * 32)
+beta_gemv1_kernel(const double* __restrict__ W, const double* __restrict__ g, double* __restrict__ tv, int p, int P,
+                  unsigned long long seed, const Ctl* __restrict__ ctl) {
+  const int row = blockIdx.x * kGemvWarps + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (row >= p) return;
+  const double* w = W + (size_t)row * P;
+  const int end = (row / CT + 1) * CT;               // W is zero right of the diagonal inside its tile
+  double s0 = 0.0, s1 = 0.0;
+  for (int c = 2 * lane; c < end; c += 64) {
+    const double2 a = *reinterpret_cast<const double2*>(w + c);
+    const double2 b = *reinterpret_cast<const double2*>(g + c);
+    s0 = fma(a.x, b.x, s0);
+    s1 = fma(a.y, b.y, s1);
+  }
+  double s = s0 + s1;
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  if (lane == 0) {
+    const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
+    tv[row] = s + norm_inv(uniform_a(seed, (unsigned long long)row, sweep, TAG_E));
+  }
+}
+
+// d2, second half: beta = Wt t (L^T beta = t), one warp per row.
+__global__ void __launch_bounds__(kGemvWarps * 32)
+beta_gemv2_kernel(const double* __restrict__ Wt, const double* __restrict__ tv, double* __restrict__ beta, int p, int P,
+                  Ctl* __restrict__ ctl) {
+  const int row = blockIdx.x * kGemvWarps + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (row >= p) return;
+  const double* w = Wt + (size_t)row * P;
+  const int begin = (row / CT) * CT;                 // Wt is zero left of the diagonal inside its tile
+  double s0 = 0.0, s1 = 0.0;
+  for (int c = begin + 2 * lane; c < P; c += 64) {
+    const double2 a = *reinterpret_cast<const double2*>(w + c);
+    const double2 b = *reinterpret_cast<const double2*>(tv + c);
+    s0 = fma(a.x, b.x, s0);
+    s1 = fma(a.y, b.y, s1);
+  }
+  double s = s0 + s1;
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  if (lane == 0) {
+    beta[row] = s;
+    if (!isfinite(s)) atomicCAS(&ctl->status, 0, -5);
+  }
+}
+
+static int env_int2(const char* name, int dflt) {
+  const char* v = getenv(name);
+  return (v && *v) ? atoi(v) : dflt;
+}
+
+// Number of CTAs for the Cholesky branch.  When the branch is expected to hide behind the fused pass
+// it gets `k` SMs of its own and the fused pass the other num_sms - k; otherwise every SM.
+int chol_plan_ctas(int p, int num_sms, double fused_ms_estimate, bool* overlap) {
+  const int nt = chol_tiles(p);
+  const double flops = 2.0 * (double)p * p * p / 3.0;             // Cholesky + inverse factor
+  const double per_sm = 0.5 * 2.0 * 64.0 * 1.9e9;                 // ~50 % of 64 DFMA/clk/SM
+  int k = env_int2("HSP_CHOL_CTAS", 0);
+  bool ov;
+  if (k > 0) {
+    ov = k < num_sms;
+  } else {
+    const double critical_ms = nt * 0.014;                        // ~14 us per tile column
+    k = 8;
+    while (k < 40 && (flops / (k * per_sm)) * 1e3 > 0.8 * fused_ms_estimate) k += 4;
+    const double t = (flops / (k * per_sm)) * 1e3;
+    ov = t <= 0.9 * fused_ms_estimate && critical_ms <= 0.9 * fused_ms_estimate;
+    if (!ov) k = num_sms;
+  }
+  const long long ntasks = (long long)nt * nt;
+  if (k > ntasks) k = (int)ntasks;
+  if (k > num_sms) k = num_sms;
+  if (overlap) *overlap = ov;
+  return k;
+}
+
+cudaError_t chol_prepare() {
+  return cudaFuncSetAttribute(chol_dataflow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCholSmem);
+}
+
+cudaError_t cholesky_launch(const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W, double* Wt,
+                            int* flags, int p, int ctas, cudaStream_t st, long long* launches) {
+  int nt = chol_tiles(p);
+  cudaError_t e = cudaMemsetAsync(flags, 0, chol_flag_count(p) * sizeof(int), st);
+  if (e != cudaSuccess) return e;
+  void* args[] = {(void*)&G, (void*)&lam_inv2, (void*)&ctl, (void*)&L, (void*)&W, (void*)&Wt, (void*)&flags, (void*)&p,
+                  (void*)&nt};
+  e = cudaLaunchCooperativeKernel((const void*)chol_dataflow_kernel, dim3(ctas), dim3(kCholThreads), args, kCholSmem, st);
+  if (launches) ++*launches;
+  return e;
+}
+
+cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g, double* tv, double* beta, int p,
+                              unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches) {
+  const int P = chol_ld(p);
+  const int grid = (p + kGemvWarps - 1) / kGemvWarps;
+  beta_gemv1_kernel<<<grid, kGemvWarps * 32, 0, st>>>(W, g, tv, p, P, seed, ctl);
+  beta_gemv2_kernel<<<grid, kGemvWarps * 32, 0, st>>>(Wt, tv, beta, p, P, ctl);
+  if (launches) *launches += 2;
   return cudaGetLastError();
 }
 

@@ -124,10 +124,10 @@ static int env_int(const char* name, int dflt) {
   return (v && *v) ? atoi(v) : dflt;
 }
 
-constexpr int kComputeWarps = 8;
+constexpr int kComputeWarps = 8;                 // compute warps per row group (they cover one row's columns)
 constexpr int kComputeThreads = kComputeWarps * 32;
 constexpr int kSamplerWarps = 4;
-constexpr int kTmaThreads = (kComputeWarps + kSamplerWarps + 1) * 32;
+__host__ __device__ constexpr int tma_threads(int G) { return (G * kComputeWarps + kSamplerWarps + 1) * 32; }
 constexpr int kFlushRows = 16;   // fp32 x*z chains are flushed into the fp64 accumulators every >= 16 rows
 
 struct TmaSmemLayout {
@@ -142,14 +142,21 @@ struct TmaSmemLayout {
   }
 };
 
-template <typename XT, int RT, int C>
-__global__ void __launch_bounds__(kTmaThreads, 1)
+// G row groups of 8 compute warps each: group g owns rows [g RT/G, (g+1) RT/G) of every tile (more
+// warps in flight per SM for the same tile shape; each group keeps its own X^T z accumulators and
+// writes its own partial row).
+template <typename XT, int RT, int C, int G>
+__global__ void __launch_bounds__(tma_threads(G), 1)
 fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
                unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
                double* __restrict__ partial, double* __restrict__ z_out, int S, int D, long long n_tiles, int dbg) {
   constexpr int V = Vec<XT>::V;
   using Acc = typename Vec<XT>::Acc;
   constexpr bool kF32 = sizeof(XT) == 4;
+  constexpr int RG = RT / G;                       // rows of a tile per group
+  constexpr int kAllCompute = G * kComputeWarps;
+  constexpr int kThreads = tma_threads(G);
+  static_assert(RT % G == 0 && RG >= 1, "rows per tile must split evenly over the groups");
   extern __shared__ __align__(128) unsigned char smem[];
   const size_t row_bytes = (size_t)p * sizeof(XT);
   const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
@@ -171,8 +178,8 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
   if (tid == 0) {
     for (int s = 0; s < S; ++s) {
       mbar_init(&full[s], 1);
-      mbar_init(&empty[s], kComputeWarps);
-      mbar_init(&eta_full[s], kComputeWarps);
+      mbar_init(&empty[s], kAllCompute);
+      mbar_init(&eta_full[s], kAllCompute);
       mbar_init(&z_full[s], 1);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -181,13 +188,13 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
   // (stale or zero) and contribute x * 0 = 0 in the xz phase, so the inner loops need no row guards.
   {
     const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
-    for (size_t o = (size_t)tid * 16; o < (size_t)S * stage_bytes; o += (size_t)kTmaThreads * 16)
+    for (size_t o = (size_t)tid * 16; o < (size_t)S * stage_bytes; o += (size_t)kThreads * 16)
       *reinterpret_cast<uint4*>(tiles + o) = zero;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes before TMA writes
   }
   __syncthreads();
 
-  if (warp == kComputeWarps + kSamplerWarps) {
+  if (warp == kAllCompute + kSamplerWarps) {
     // ===================== producer: one thread streams the tiles =====================
     if (lane == 0) {
       int st = 0;
@@ -203,11 +210,11 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         if (++st == S) { st = 0; ph ^= 1u; }
       }
     }
-  } else if (warp >= kComputeWarps) {
+  } else if (warp >= kAllCompute) {
     // ===================== sampler warps: eta -> z, D tiles behind the eta phase =====================
     // Tile n goes to sampler warp n mod ns.  ns <= S keeps every mbarrier wait at most one phase
     // behind (a waiter two phases behind would alias on the parity bit).
-    const int sw = warp - kComputeWarps;
+    const int sw = warp - kAllCompute;
     const int ns = S < kSamplerWarps ? S : kSamplerWarps;
     if (sw < ns) {
       // y is prefetched three tiles ahead: under a saturated HBM a lone 1-byte load takes microseconds
@@ -248,15 +255,16 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     }
   } else {
     // ===================== compute warps: eta partials, then x*z from the same stage =====================
-    // Thread t owns the 16-byte column stripes (c*256 + t)*V.  Stripes past p read column 0 with
-    // beta = 0 and are never written back, so the loops below are straight-line code.
+    // Thread t of a group owns the 16-byte column stripes (c*256 + t)*V.  Stripes past p read column 0
+    // with beta = 0 and are never written back, so the loops below are straight-line code.
+    const int grp = warp / kComputeWarps, wg = warp % kComputeWarps, gt = tid % kComputeThreads;
     double breg[C][V];
     double acc64[C][V];
     Acc acc[C][V];
     uint32_t coff[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) {
-      const int col = (c * kComputeThreads + tid) * V;
+      const int col = (c * kComputeThreads + gt) * V;
       coff[c] = (col < p) ? (uint32_t)(col * sizeof(XT)) : 0u;
 #pragma unroll
       for (int v = 0; v < V; ++v) {
@@ -265,9 +273,10 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         acc[c][v] = (Acc)0;
       }
     }
-    const int my_row = row_of_lane<RT>(lane);
-    const bool writer = (lane & (32 / RT - 1)) == 0;
+    const int my_row = grp * RG + row_of_lane<RG>(lane);
+    const bool writer = (lane & (32 / RG - 1)) == 0;
     const uint32_t rb = (uint32_t)row_bytes;
+    const uint32_t goff = (uint32_t)(grp * RG) * rb;   // first row of this group inside a tile
     int rows_since_flush = 0;
     int st_e = 0, st_g = 0;
     uint32_t ph_e = 0, ph_g = 0;
@@ -275,49 +284,49 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     for (int it = 0; it < total_it; ++it) {
       if (it < (int)my_tiles) {
         mbar_wait(&full[st_e], ph_e);
-        const unsigned char* tile = tiles + (size_t)st_e * stage_bytes;
-        double part[RT];
+        const unsigned char* tile = tiles + (size_t)st_e * stage_bytes + goff;
+        double part[RG];
 #pragma unroll
-        for (int r = 0; r < RT; ++r) part[r] = 0.0;
+        for (int r = 0; r < RG; ++r) part[r] = 0.0;
         if (!(dbg & 2)) {
 #pragma unroll
           for (int c = 0; c < C; ++c) {
-            Vec<XT> x[RT];
+            Vec<XT> x[RG];
 #pragma unroll
-            for (int r = 0; r < RT; ++r) x[r].load(tile + r * rb + coff[c]);
+            for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
 #pragma unroll
-            for (int r = 0; r < RT; ++r) part[r] += x[r].dot(breg[c]);
+            for (int r = 0; r < RG; ++r) part[r] += x[r].dot(breg[c]);
           }
         }
-        const double tot = warp_reduce_rows<RT>(part, lane);
-        if (writer) eta_part[((size_t)st_e * kComputeWarps + warp) * RT + my_row] = tot;
+        const double tot = warp_reduce_rows<RG>(part, lane);
+        if (writer) eta_part[((size_t)st_e * kComputeWarps + wg) * RT + my_row] = tot;
         __syncwarp();
         if (lane == 0) mbar_arrive(&eta_full[st_e]);
         if (++st_e == S) { st_e = 0; ph_e ^= 1u; }
       }
       if (it >= D) {
         mbar_wait(&z_full[st_g], ph_g);
-        const unsigned char* tile = tiles + (size_t)st_g * stage_bytes;
-        Acc zr[RT];
+        const unsigned char* tile = tiles + (size_t)st_g * stage_bytes + goff;
+        Acc zr[RG];
         if constexpr (kF32) {
-          const float* zp = z32 + st_g * RT;
-          if constexpr (RT % 4 == 0) {
+          const float* zp = z32 + st_g * RT + grp * RG;
+          if constexpr (RG % 4 == 0) {
 #pragma unroll
-            for (int q = 0; q < RT / 4; ++q) {
+            for (int q = 0; q < RG / 4; ++q) {
               const float4 t = *reinterpret_cast<const float4*>(zp + 4 * q);
               zr[4 * q] = t.x; zr[4 * q + 1] = t.y; zr[4 * q + 2] = t.z; zr[4 * q + 3] = t.w;
             }
-          } else if constexpr (RT == 2) {
+          } else if constexpr (RG == 2) {
             const float2 t = *reinterpret_cast<const float2*>(zp);
             zr[0] = t.x; zr[1] = t.y;
           } else {
             zr[0] = zp[0];
           }
         } else {
-          const double* zp = z64 + st_g * RT;
-          if constexpr (RT % 2 == 0) {
+          const double* zp = z64 + st_g * RT + grp * RG;
+          if constexpr (RG % 2 == 0) {
 #pragma unroll
-            for (int q = 0; q < RT / 2; ++q) {
+            for (int q = 0; q < RG / 2; ++q) {
               const double2 t = *reinterpret_cast<const double2*>(zp + 2 * q);
               zr[2 * q] = t.x; zr[2 * q + 1] = t.y;
             }
@@ -328,18 +337,18 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         if (!(dbg & 4)) {
 #pragma unroll
           for (int c = 0; c < C; ++c) {
-            Vec<XT> x[RT];
+            Vec<XT> x[RG];
 #pragma unroll
-            for (int r = 0; r < RT; ++r) x[r].load(tile + r * rb + coff[c]);
+            for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
 #pragma unroll
-            for (int r = 0; r < RT; ++r) x[r].axpy(zr[r], acc[c]);
+            for (int r = 0; r < RG; ++r) x[r].axpy(zr[r], acc[c]);
           }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st_g]);
         if (++st_g == S) { st_g = 0; ph_g ^= 1u; }
         if constexpr (kF32) {
-          rows_since_flush += RT;
+          rows_since_flush += RG;
           if (rows_since_flush >= kFlushRows) {
             rows_since_flush = 0;
 #pragma unroll
@@ -352,10 +361,10 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     }
 #pragma unroll
     for (int c = 0; c < C; ++c) {
-      const int col = (c * kComputeThreads + tid) * V;
+      const int col = (c * kComputeThreads + gt) * V;
 #pragma unroll
       for (int v = 0; v < V; ++v)
-        if (col + v < p) partial[(size_t)cta * p + col + v] = acc64[c][v] + (double)acc[c][v];
+        if (col + v < p) partial[((size_t)cta * G + grp) * p + col + v] = acc64[c][v] + (double)acc[c][v];
     }
   }
 }
@@ -440,13 +449,24 @@ fused_pass_generic(const XT* __restrict__ X, const unsigned char* __restrict__ y
   }
 }
 
-// b: g_j = sum_c partial[c][j], c ascending (no float atomics)
-__global__ void reduce_partials_kernel(const double* __restrict__ partial, int n_part, int p, double* __restrict__ g) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= p) return;
+// b: g_j = sum_c partial[c][j] in a fixed order (no float atomics): 32 columns per CTA; thread (x, y)
+// adds rows y, y+32, ... of column x, then row 0 adds the 32 sub-sums in ascending y.
+__global__ void __launch_bounds__(1024)
+reduce_partials_kernel(const double* __restrict__ partial, int n_part, int p, double* __restrict__ g) {
+  __shared__ double red[32][33];
+  const int x = threadIdx.x, y = threadIdx.y;
+  const int j = blockIdx.x * 32 + x;
   double s = 0.0;
-  for (int c = 0; c < n_part; ++c) s += partial[(size_t)c * p + j];
-  g[j] = s;
+  if (j < p)
+    for (int c = y; c < n_part; c += 32) s += partial[(size_t)c * p + j];
+  red[y][x] = s;
+  __syncthreads();
+  if (y == 0 && j < p) {
+    double t = 0.0;
+#pragma unroll
+    for (int q = 0; q < 32; ++q) t += red[q][x];
+    g[j] = t;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -486,10 +506,14 @@ FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X) 
       if (D < 1) D = 1;
       pl.variant = 1;
       pl.rows_per_tile = RT; pl.chunks = C; pl.stages = S; pl.lag = D;
+      int G = env_int("HSP_FUSED_GROUPS", 2);
+      if (G != 1 && G != 2) G = 2;
+      if (RT % G != 0) G = 1;
+      pl.groups = G;
       pl.n_tiles = (N + RT - 1) / RT;
       int grid = env_int("HSP_FUSED_GRID", num_sms);
       if ((long long)grid > pl.n_tiles) grid = (int)pl.n_tiles;
-      pl.grid = grid; pl.block = kTmaThreads;
+      pl.grid = grid; pl.block = tma_threads(G);
       pl.smem = TmaSmemLayout(S, RT, stage_bytes).total;
       return pl;
     }
@@ -499,15 +523,15 @@ FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X) 
   long long grid = (long long)num_sms * 4;
   if (grid > pl.n_tiles) grid = pl.n_tiles;
   pl.grid = (int)grid; pl.block = kGenThreads; pl.smem = 0;
-  pl.rows_per_tile = kGenThreads; pl.chunks = 0; pl.stages = 0; pl.lag = 0;
+  pl.rows_per_tile = kGenThreads; pl.chunks = 0; pl.stages = 0; pl.lag = 0; pl.groups = 1;
   return pl;
 }
 
-template <typename XT, int RT, int C>
+template <typename XT, int RT, int C, int G>
 static cudaError_t launch_tma(const FusedPlan& pl, const void* X, const unsigned char* y, long long N, int p,
                               unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                               double* z_out, cudaStream_t st) {
-  auto kern = fused_pass_tma<XT, RT, C>;
+  auto kern = fused_pass_tma<XT, RT, C, G>;
   static bool configured = false;   // per instantiation
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
@@ -524,16 +548,23 @@ template <typename XT>
 static cudaError_t dispatch_tma(const FusedPlan& pl, const void* X, const unsigned char* y, long long N, int p,
                                 unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                                 double* z_out, cudaStream_t st) {
+#define HSP_TMA_CASE(RT_, C_)                                                                              \
+  case C_:                                                                                                 \
+    if constexpr ((RT_) % 2 == 0) {                                                                        \
+      if (pl.groups == 2) return launch_tma<XT, RT_, C_, 2>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st); \
+    }                                                                                                      \
+    return launch_tma<XT, RT_, C_, 1>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
   switch (pl.chunks) {
-    case 1: return launch_tma<XT, 8, 1>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
-    case 2: return launch_tma<XT, 4, 2>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
-    case 3: return launch_tma<XT, 2, 3>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
-    case 4: return launch_tma<XT, 2, 4>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
-    case 6: return launch_tma<XT, 1, 6>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
-    case 8: return launch_tma<XT, 1, 8>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
-    case 12: return launch_tma<XT, 1, 12>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
-    case 16: return launch_tma<XT, 1, 16>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+    HSP_TMA_CASE(8, 1)
+    HSP_TMA_CASE(4, 2)
+    HSP_TMA_CASE(2, 3)
+    HSP_TMA_CASE(2, 4)
+    HSP_TMA_CASE(1, 6)
+    HSP_TMA_CASE(1, 8)
+    HSP_TMA_CASE(1, 12)
+    HSP_TMA_CASE(1, 16)
   }
+#undef HSP_TMA_CASE
   return cudaErrorInvalidValue;
 }
 
@@ -557,7 +588,7 @@ cudaError_t fused_pass_launch(const FusedPlan& pl, const void* X, int dtype, con
 }
 
 cudaError_t reduce_partials_launch(const double* partial, int n_part, int p, double* g, cudaStream_t st) {
-  reduce_partials_kernel<<<(p + 127) / 128, 128, 0, st>>>(partial, n_part, p, g);
+  reduce_partials_kernel<<<(p + 31) / 32, dim3(32, 32), 0, st>>>(partial, n_part, p, g);
   return cudaGetLastError();
 }
 

@@ -35,8 +35,9 @@ struct hsp_state {
   cudaStream_t own_stream = nullptr;
   unsigned flags = 0; int num_sms = 0;
   void* own_X = nullptr; unsigned char* own_y = nullptr;
-  double *G = nullptr, *L = nullptr, *beta = nullptr, *lam_inv2 = nullptr, *nu_inv = nullptr, *g = nullptr,
-         *partial = nullptr, *z = nullptr;
+  double *G = nullptr, *L = nullptr, *W = nullptr, *Wt = nullptr, *beta = nullptr, *lam_inv2 = nullptr,
+         *nu_inv = nullptr, *g = nullptr, *tv = nullptr, *partial = nullptr, *z = nullptr;
+  int* chol_flags = nullptr; int chol_ctas = 0; bool chol_overlap = false;
   signed char* side = nullptr;
   Ctl* ctl = nullptr;
   double *h_beta = nullptr, *h_lambda = nullptr, *h_tau = nullptr;
@@ -58,8 +59,8 @@ static void free_state(hsp_state* s) {
   if (s->ev_join) cudaEventDestroy(s->ev_join);
   if (s->stream2) cudaStreamDestroy(s->stream2);
   if (s->own_stream) cudaStreamDestroy(s->own_stream);
-  void* ptrs[] = {s->own_X, s->own_y, s->G, s->L, s->beta, s->lam_inv2, s->nu_inv, s->g, s->partial, s->z, s->side,
-                  s->ctl, s->h_beta, s->h_lambda, s->h_tau};
+  void* ptrs[] = {s->own_X, s->own_y, s->G, s->L, s->W, s->Wt, s->beta, s->lam_inv2, s->nu_inv, s->g, s->tv, s->partial,
+                  s->z, s->side, s->chol_flags, s->ctl, s->h_beta, s->h_lambda, s->h_tau};
   for (void* q : ptrs) if (q) cudaFree(q);
   delete s;
 }
@@ -96,19 +97,18 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
     CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, s->N, s->p, s->seed, s->beta, s->ctl, s->partial,
                          (s->flags & HSP_STORE_Z) ? s->z : nullptr, A));
     if (timed) { CK(cudaEventRecord(s->tev[s->tev_used + 1], A)); s->tev_used += 2; }
-    CK(reduce_partials_launch(s->partial, s->plan.grid, s->p, s->g, A));
+    CK(reduce_partials_launch(s->partial, s->plan.grid * s->plan.groups, s->p, s->g, A));
     *kernels += 2;
   }
   if (do_scales) { CK(scales_pre_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, B)); *kernels += 1; }
   if (do_beta) {
-    CK(build_q_launch(s->G, s->lam_inv2, s->ctl, s->L, s->p, B)); *kernels += 1;
-    CK(cholesky_launch(s->L, s->p, s->ctl, B, kernels));
+    CK(cholesky_launch(s->G, s->lam_inv2, s->ctl, s->L, s->W, s->Wt, s->chol_flags, s->p, s->chol_ctas, B, kernels));
   }
   if (!serial && side_work) {
     CK(cudaEventRecord(s->ev_join, B));
     CK(cudaStreamWaitEvent(A, s->ev_join, 0));
   }
-  if (do_beta) { CK(beta_draw_launch(s->L, s->g, s->beta, s->p, s->seed, s->ctl, A)); *kernels += 1; }
+  if (do_beta) CK(beta_solve_launch(s->W, s->Wt, s->g, s->tv, s->beta, s->p, s->seed, s->ctl, A, kernels));
   CK(scales_post_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, do_scales ? 0 : 1, A));
   *kernels += 1;
   return HSP_OK;
@@ -144,14 +144,23 @@ static int create_common(hsp_state** out, hsp_state* s) {
   CK(cudaStreamCreateWithFlags(&s->stream2, cudaStreamNonBlocking));
   CK(cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming));
   CK(cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming));
-  s->plan = fused_plan(s->dtype, N, p, s->num_sms, s->X);
+  // SM budget: when the Cholesky branch (c, d1) can hide behind the fused pass it gets chol_ctas SMs of
+  // its own and the pass the rest; otherwise both use every SM and run one after the other.
+  const double x_bytes = (double)N * p * (s->dtype == HSP_F32 ? 4.0 : 8.0);
+  const double fused_ms_est = x_bytes / 6.0e9 + 0.01;
+  s->chol_ctas = chol_plan_ctas(p, s->num_sms, fused_ms_est, &s->chol_overlap);
+  const int fused_sms = s->chol_overlap ? s->num_sms - s->chol_ctas : s->num_sms;
+  s->plan = fused_plan(s->dtype, N, p, fused_sms, s->X);
   // set opt-in shared-memory attributes now, outside any stream capture
   CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, -1, p, 0, nullptr, nullptr, nullptr, nullptr, s->stream));
-  CK(beta_draw_launch(nullptr, nullptr, nullptr, p, 0, nullptr, s->stream));
+  CK(chol_prepare());
   const size_t pp = (size_t)p * p * sizeof(double), pv = (size_t)p * sizeof(double);
-  CK(cudaMalloc(&s->G, pp)); CK(cudaMalloc(&s->L, pp));
-  CK(cudaMalloc(&s->beta, pv)); CK(cudaMalloc(&s->lam_inv2, pv)); CK(cudaMalloc(&s->nu_inv, pv)); CK(cudaMalloc(&s->g, pv));
-  CK(cudaMalloc(&s->partial, (size_t)s->plan.grid * pv));
+  const size_t P = (size_t)chol_ld(p), PP = P * P * sizeof(double), Pv = P * sizeof(double);
+  CK(cudaMalloc(&s->G, pp)); CK(cudaMalloc(&s->L, PP)); CK(cudaMalloc(&s->W, PP)); CK(cudaMalloc(&s->Wt, PP));
+  CK(cudaMalloc(&s->chol_flags, chol_flag_count(p) * sizeof(int)));
+  CK(cudaMalloc(&s->beta, pv)); CK(cudaMalloc(&s->lam_inv2, pv)); CK(cudaMalloc(&s->nu_inv, pv));
+  CK(cudaMalloc(&s->g, Pv)); CK(cudaMalloc(&s->tv, Pv));     // padded to P with zeros (the GEMVs read whole tiles)
+  CK(cudaMalloc(&s->partial, (size_t)s->plan.grid * s->plan.groups * pv));
   CK(cudaMalloc(&s->ctl, sizeof(Ctl)));
   // validate y in {0,1}
   int* bad = nullptr;
@@ -167,7 +176,9 @@ static int create_common(hsp_state** out, hsp_state* s) {
   // cold start: beta = 0; lambda = nu = tau = xi = 1
   std::vector<double> ones((size_t)p, 1.0);
   CK(cudaMemsetAsync(s->beta, 0, pv, s->stream));
-  CK(cudaMemsetAsync(s->g, 0, pv, s->stream));
+  CK(cudaMemsetAsync(s->g, 0, Pv, s->stream));
+  CK(cudaMemsetAsync(s->tv, 0, Pv, s->stream));
+  CK(cudaMemsetAsync(s->L, 0, PP, s->stream));
   CK(cudaMemcpyAsync(s->lam_inv2, ones.data(), pv, cudaMemcpyHostToDevice, s->stream));
   CK(cudaMemcpyAsync(s->nu_inv, ones.data(), pv, cudaMemcpyHostToDevice, s->stream));
   Ctl c{}; c.sweep = 0; c.hist_base = 0; c.tau_inv2 = 1.0; c.xi_inv = 1.0; c.status = 0;
@@ -176,7 +187,7 @@ static int create_common(hsp_state** out, hsp_state* s) {
   CK(cudaStreamSynchronize(s->stream));   // `ones` and `c` are stack/heap temporaries
   // c0: G = X^T X once
   const int splits = gram_splits(N, p, s->num_sms);
-  double* scratch = s->L;                  // L is free until the first sweep
+  double* scratch = s->W;                  // W (>= p*p doubles) is free until the first sweep
   if (splits > 1) CK(cudaMalloc(&scratch, (size_t)splits * pp));
   cudaError_t e = gram_launch(s->X, s->dtype, N, p, s->G, scratch, splits, s->stream);
   s->launches += 3;
@@ -399,7 +410,8 @@ int hsp_get_gram(const hsp_state* s, double* G) {
 int hsp_get_chol(const hsp_state* s, double* L) {
   if (!s || !L) return fail(HSP_EINVAL, "NULL argument");
   CK(cudaStreamSynchronize(s->stream));
-  CK(cudaMemcpy(L, s->L, (size_t)s->p * s->p * sizeof(double), cudaMemcpyDefault));
+  const size_t rb = (size_t)s->p * sizeof(double);
+  CK(cudaMemcpy2D(L, rb, s->L, (size_t)chol_ld(s->p) * sizeof(double), rb, (size_t)s->p, cudaMemcpyDefault));
   return HSP_OK;
 }
 

@@ -28,11 +28,12 @@ struct FusedPlan {
   int stages;         // S
   int lag;            // D
   int chunks;         // C
+  int groups;         // G: row groups of compute warps (partial rows = grid * G)
   long long n_tiles;
 };
 
 // ---- fused pass (a1-a3) and reduce (b): fused_pass.cu
-FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X);
+FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X);   // num_sms: CTAs the pass may use
 cudaError_t fused_pass_launch(const FusedPlan& plan, const void* X, int dtype, const unsigned char* y, long long N,
                               int p, unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                               double* z_out, cudaStream_t st);
@@ -43,11 +44,16 @@ cudaError_t gram_launch(const void* X, int dtype, long long N, int p, double* G,
                         cudaStream_t st);
 int gram_splits(long long N, int p, int num_sms);
 
-// ---- Q build (c), Cholesky (d1), beta draw (d2): cholesky.cu
-cudaError_t build_q_launch(const double* G, const double* lam_inv2, const Ctl* ctl, double* L, int p, cudaStream_t st);
-cudaError_t cholesky_launch(double* L, int p, Ctl* ctl, cudaStream_t st, long long* launches);
-cudaError_t beta_draw_launch(const double* L, const double* g, double* beta, int p, unsigned long long seed,
-                             Ctl* ctl, cudaStream_t st);
+// ---- Q build (c), Cholesky + inverse factor (d1), beta draw (d2): cholesky.cu
+int chol_tiles(int p);                 // nt = ceil(p / 64)
+int chol_ld(int p);                    // P = 64 nt: leading dimension of L, W, Wt (padded with the identity)
+size_t chol_flag_count(int p);         // ints of per-tile "done" flags
+int chol_plan_ctas(int p, int num_sms, double fused_ms_estimate, bool* overlap);
+cudaError_t chol_prepare();
+cudaError_t cholesky_launch(const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W, double* Wt,
+                            int* flags, int p, int ctas, cudaStream_t st, long long* launches);
+cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g, double* tv, double* beta, int p,
+                              unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches);
 
 // ---- scale conditionals (e1, e2, e3) and draw output (g): scales.cu
 cudaError_t scales_pre_launch(const double* beta, double* lam_inv2, const double* nu_inv, Ctl* ctl, int p,
