@@ -397,10 +397,12 @@ int chol_plan_ctas(int p, int num_sms, double fused_ms_estimate, bool* overlap) 
   if (k > 0) {
     ov = k < num_sms;
   } else {
-    const double critical_ms = nt * 0.014;                        // ~14 us per tile column
+    // measured on B200 (profiles/r01_b): the left-looking task chain costs ~35 us per tile column, and the
+    // kernel takes ~2.6x the time the flop count at 50 % of the DFMA rate suggests
+    const double critical_ms = nt * 0.035;
     k = 8;
-    while (k < 40 && (flops / (k * per_sm)) * 1e3 > 0.8 * fused_ms_estimate) k += 4;
-    const double t = (flops / (k * per_sm)) * 1e3;
+    while (k < 48 && 2.6 * (flops / (k * per_sm)) * 1e3 > 0.85 * fused_ms_estimate) k += 4;
+    const double t = 2.6 * (flops / (k * per_sm)) * 1e3;
     ov = t <= 0.9 * fused_ms_estimate && critical_ms <= 0.9 * fused_ms_estimate;
     if (!ov) k = num_sms;
   }
