@@ -50,7 +50,7 @@ class ClockSampler:
     def __enter__(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE, text=True)
+                                          "--format=csv,noheader,nounits", "-lms", "20"], stdout=subprocess.PIPE, text=True)
             self.thread = threading.Thread(target=lambda: [self.lines.append(l) for l in self.proc.stdout], daemon=True)
             self.thread.start()
         except OSError:
@@ -190,6 +190,7 @@ def main():
         fused_ms, fused_n = chain.fused_pass_ms()
         launches = chain.launch_count() - k0
         variant = chain.fused_variant()
+        plan = chain.plan()
         # sanity: the chain is finite and moving
         b, lam, tau = chain.get_draws()
         assert np.all(np.isfinite(b)) and np.all(np.isfinite(lam)) and np.all(tau > 0)
@@ -221,7 +222,7 @@ def main():
                 "vs_baseline": value / PAPER_SWEEPS_PER_S if args.workload == "C3" else None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": WORKLOAD_DESC[args.workload], "x_dtype": str(wl.X.dtype).replace("torch.", ""),
-                           "positive_rate": wl.positive_rate, "fused_kernel": variant,
+                           "positive_rate": wl.positive_rate, "fused_kernel": variant, "plan": plan,
                            "l2": "X (%.1f GB) is larger than L2 and is streamed once per step" % (x_bytes / 1e9)
                            if x_bytes > 256e6 else "inputs fit L2: latency-bound config, absolute number only",
                            "launch_mode": "cuda-graph replay" if args.graph else "direct launches, 2 streams",

@@ -114,6 +114,10 @@ int hsp_get_chol(const hsp_state* s, double* L);
 int hsp_get_fused_pass_ms(hsp_state* s, double* ms, long long* launches);
 /* Number of kernels this library launched (directly or through graph replays) since create.      */
 long long hsp_get_launch_count(const hsp_state* s);
+/* Launch plan chosen at create: CTAs of the fused pass (a1-a3), CTAs of the Cholesky branch (c, d1),
+ * whether the two run side by side on disjoint SMs (1) or one after the other (0), and the cost-model
+ * estimate of the Cholesky branch in microseconds.  HOST pointers, any may be NULL.               */
+int hsp_get_plan(const hsp_state* s, int* fused_ctas, int* chol_ctas, int* overlap, double* chol_est_us);
 /* Name of the fused-pass kernel variant selected for this (dtype, p): "tma" or "generic".        */
 const char* hsp_fused_variant(const hsp_state* s);
 
@@ -128,6 +132,15 @@ int hsp_dbg_uniform(unsigned long long seed, const unsigned long long* idx, unsi
 int hsp_dbg_tnpos(const double* m, const double* u, double* w, long long n, void* stream);
 int hsp_dbg_norm_inv(const double* u, double* x, long long n, void* stream);
 int hsp_dbg_cheng(double alpha, unsigned long long seed, unsigned sweep0, double* x, long long n, void* stream);
+
+
+/* Measurement hook for rows c, d1: the static schedule of the Cholesky task graph and, if
+ * the environment variable HSP_CHOL_TRACE=1 was set when the chain was created, the device timestamps of
+ * the tasks of the last sweep.  rows: HOST, capacity x 12 long long per task, in schedule order:
+ * {type, i, j, kbeg, kend, slot_in, slot_out, cta, t_start_ns, t_kloop_end_ns, t_end_ns, 0} (timestamps 0
+ * without the trace).  Returns the number of tasks (rows may be NULL to query it), or a negative status.
+ * Synchronises.                                                                                     */
+long long hsp_dbg_chol_trace(const hsp_state* s, long long* rows, long long capacity);
 
 #ifdef __cplusplus
 }

@@ -66,6 +66,9 @@ def lib():
     L.hsp_dbg_tnpos.argtypes = [vp, vp, vp, ll, vp]
     L.hsp_dbg_norm_inv.argtypes = [vp, vp, ll, vp]
     L.hsp_dbg_cheng.argtypes = [C.c_double, ull, C.c_uint, vp, ll, vp]
+    L.hsp_dbg_chol_trace.argtypes = [vp, vp, ll]
+    L.hsp_get_plan.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), dp]
+    L.hsp_dbg_chol_trace.restype = ll
     _lib = L
     return L
 
@@ -186,6 +189,22 @@ class HorseshoeProbit:
 
     def fused_variant(self):
         return lib().hsp_fused_variant(self._h).decode()
+
+    def plan(self):
+        a, b, c, d = C.c_int(), C.c_int(), C.c_int(), C.c_double()
+        _check(lib().hsp_get_plan(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(d)))
+        return {"fused_ctas": a.value, "chol_ctas": b.value, "overlap": bool(c.value), "chol_est_us": d.value}
+
+    def chol_trace(self):
+        """Static tile schedule of rows c, d1 (and timestamps, with HSP_CHOL_TRACE=1): int64 [n_tasks, 12]."""
+        n = lib().hsp_dbg_chol_trace(self._h, None, 0)
+        if n < 0:
+            _check(int(n))
+        rows = np.zeros((n, 12), dtype=np.int64)
+        n2 = lib().hsp_dbg_chol_trace(self._h, _np(rows), n)
+        if n2 < 0:
+            _check(int(n2))
+        return rows
 
 
 # ---- device unit-test hooks (torch CUDA tensors in, torch CUDA tensors out) -------------------------

@@ -3,8 +3,8 @@
 //   d1  Q = L L^T, tiled fp64 Cholesky
 //   d2  beta = Q^-1 g + L^-T e,  e_j = Phi^-1(u_j)           PAPER.md:180, 198-202, 239 (reading R5)
 //
-// One persistent kernel (`chol_dataflow_kernel`) does c and d1 and, in the same task graph, the inverse
-// factor W = L^-1 (and its transpose Wt = L^-T): d2 then needs no substitution on the critical path
+// One persistent cooperative kernel (`chol_task_kernel`) does c and d1 and, in the same task graph, the
+// inverse factor W = L^-1 (and its transpose Wt = L^-T): d2 then needs no substitution on the critical path
 // after X^T z arrives -- it is two triangular matrix-vector products, t = W g + e and beta = Wt t,
 // i.e. L t = g + L e and L^T beta = t, exactly the two solves of PAPER.md:199-201.
 //
@@ -12,33 +12,38 @@
 //   L(i,j), i >= j :  A = Q_ij - sum_{k<j} L_ik L_jk^T ;  i == j: L_jj = chol(A), W_jj = L_jj^-1 ;
 //                                                         i >  j: L_ij = A W_jj^T
 //   B(i,j), i <  j :  A = - sum_{k=i}^{j-1} L_jk Wt_ik^T ; W_ji = W_jj A  (stored in W and, transposed, in Wt)
-// Tasks are numbered column by column and dealt round-robin to the CTAs; every task depends only on
-// lower-numbered tasks, each CTA runs its tasks in order, and all CTAs are co-resident (cooperative
-// launch), so spinning on the per-tile "done" flags cannot deadlock.  Every tile is computed by one
-// CTA with a fixed summation order: the result does not depend on the number of CTAs.
+// The host (chol_schedule.cu) splits the tiles on the critical path into prefix + finish tasks and deals all
+// tasks to the CTAs as static ordered lists; a CTA runs its list in order and waits on per-tile "done" flags
+// inside the k-loop.  All CTAs are co-resident (cooperative launch) and every list is a subsequence of one
+// global order in which producers precede consumers, so the spin-waits cannot deadlock.  Every tile is
+// accumulated in ascending k by a fixed sequence of tasks: the result does not depend on the number of CTAs.
+//
+// Tile products run on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> SASS DMMA; tcgen05 has no f64 kind):
+// 8 warps x (32 rows x 16 columns) of the 64x64 accumulator, operands staged by a 3-stage cp.async pipeline
+// in 32-column chunks with a padded row stride that makes the fragment loads conflict-free.
 //
 // Storage: row-major, leading dimension P; L lower, W lower, Wt upper.
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <cstdlib>
+#include <vector>
 #include "hsp_device.cuh"
 #include "hsp_internal.h"
 
 namespace hsp {
 
 constexpr int CT = 64;                 // tile edge
-constexpr int KC = 16;                 // k-columns per pipeline chunk
-constexpr int CLD = KC + 2;            // chunk row stride in doubles (144 B): conflict-free LDS.128
-constexpr int TLD = CT + 2;            // full-tile row stride in shared memory (528 B)
-constexpr int NST = 4;                 // cp.async pipeline stages
+constexpr int KC = 32;                 // k-columns per pipeline chunk
+constexpr int CLD = KC + 4;            // chunk row stride in doubles (288 B): conflict-free 64-bit fragment loads
+constexpr int TLD = CT + 4;            // full-tile row stride in shared memory (544 B)
+constexpr int NST = 3;                 // cp.async pipeline stages
 constexpr int kCholThreads = 256;
 constexpr int kStageDoubles = 2 * CT * CLD;                       // A chunk + B chunk
-constexpr size_t kCholSmem = (size_t)NST * kStageDoubles * sizeof(double) + 1024;   // 73728 + scratch
-static_assert((size_t)NST * kStageDoubles >= 2 * (size_t)CT * TLD, "finalize tiles must fit in the pipeline pool");
+constexpr int kPoolDoubles = NST * kStageDoubles;
+constexpr size_t kCholSmem = (size_t)(kPoolDoubles + 2 * CT * TLD + CT) * sizeof(double);   // pool + S + X + rdiag
 
 int chol_tiles(int p) { return (p + CT - 1) / CT; }
 int chol_ld(int p) { return chol_tiles(p) * CT; }
-size_t chol_flag_count(int p) { const size_t nt = chol_tiles(p); return 2 * nt * nt; }
 
 __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
@@ -56,172 +61,280 @@ __device__ __forceinline__ int ld_acquire(const int* p) {
 __device__ __forceinline__ void st_release(int* p, int v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
 __device__ __forceinline__ void wait_flag(const int* f) {
-  while (ld_acquire(f) == 0) __nanosleep(32);
+  while (ld_acquire(f) == 0) __nanosleep(20);
 }
 
-// acc[a][b] (rows ty+16a, cols tx+16b) += sgn * sum_k A[row][k] B[col][k],  k in [0, K), K even.
+// D(8x8) += A(8x4) B(4x8) on the FP64 tensor pipe.  Fragments (PTX ISA, m8n8k4 .f64): with g = lane / 4,
+// t = lane % 4:  a = A[g][t],  b = B[t][g],  c0,c1 = C[g][2t], C[g][2t+1].
+__device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+// Accumulator layout of one thread: warp w covers rows wm*32..+32 (wm = w & 1) and columns wn*16..+16
+// (wn = w >> 1); acc[mb][nb][e] is element (wm*32 + mb*8 + g, wn*16 + nb*8 + 2t + e).
+struct Frag {
+  int row0, col0, g, t;
+  __device__ __forceinline__ explicit Frag(int tid) {
+    const int w = tid >> 5, lane = tid & 31;
+    row0 = (w & 1) * 32; col0 = (w >> 1) * 16; g = lane >> 2; t = lane & 3;
+  }
+};
+
+// acc[m][n] += sgn * sum_k A[m][k] B[n][k],  k in [0, K): A and B are row-major [row][k] in shared memory.
 template <int LDA, int LDB, int K, bool NEG>
-__device__ __forceinline__ void tile_mac(const double* __restrict__ A, const double* __restrict__ B, int ty, int tx,
-                                         double (&acc)[4][4]) {
+__device__ __forceinline__ void tile_mma(const double* __restrict__ A, const double* __restrict__ B, const Frag& f,
+                                         double (&acc)[4][2][2]) {
+  const double* ap = A + (f.row0 + f.g) * LDA + f.t;
+  const double* bp = B + (f.col0 + f.g) * LDB + f.t;
 #pragma unroll
-  for (int kk = 0; kk < K; kk += 2) {
-    double2 av[4], bv[4];
+  for (int kk = 0; kk < K; kk += 4) {
+    double a[4], b[2];
 #pragma unroll
-    for (int a = 0; a < 4; ++a) av[a] = *reinterpret_cast<const double2*>(A + (ty + 16 * a) * LDA + kk);
+    for (int mb = 0; mb < 4; ++mb) { a[mb] = ap[mb * 8 * LDA + kk]; if (NEG) a[mb] = -a[mb]; }
 #pragma unroll
-    for (int b = 0; b < 4; ++b) bv[b] = *reinterpret_cast<const double2*>(B + (tx + 16 * b) * LDB + kk);
+    for (int nb = 0; nb < 2; ++nb) b[nb] = bp[nb * 8 * LDB + kk];
 #pragma unroll
-    for (int a = 0; a < 4; ++a)
+    for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        if (NEG) {
-          acc[a][b] = fma(-av[a].x, bv[b].x, acc[a][b]);
-          acc[a][b] = fma(-av[a].y, bv[b].y, acc[a][b]);
-        } else {
-          acc[a][b] = fma(av[a].x, bv[b].x, acc[a][b]);
-          acc[a][b] = fma(av[a].y, bv[b].y, acc[a][b]);
-        }
-      }
+      for (int nb = 0; nb < 2; ++nb) dmma(acc[mb][nb], a[mb], b[nb]);
   }
 }
 
-// In-place Cholesky of the 64x64 tile S (stride TLD, lower triangle used), all 256 threads.  On return
-// S holds L (lower, diagonal included; the strict upper triangle is zeroed).  One barrier per pivot:
-// the trailing update uses the unscaled column, S[r][c] -= S[r][j] S[c][j] / d_j, and the columns are
-// scaled by 1/sqrt(d_j) at the end.  Returns false if a pivot is not positive (then d_j := 1).
-__device__ __forceinline__ bool tile_potrf(double* __restrict__ S, double* __restrict__ dsq, int tid, int ty, int tx) {
+// 1/d for a positive normal d: MUFU seed (rcp.approx.ftz.f64, relative error e ~ 2^-20) and one cubic
+// correction r (1 + e + e^2), three dependent FMAs; the result is within ~1 ulp.
+__device__ __forceinline__ double fast_rcp(double d) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+  const double e = fma(-d, r, 1.0);
+  const double t = fma(e, e, e);
+  return fma(r, t, r);
+}
+
+// In-place Cholesky of the 64x64 tile S (stride TLD, lower triangle used), all 256 threads; on return the
+// lower triangle of S holds L (diagonal included) and rdiag[r] = 1 / L_rr.  Blocked by 16 columns: the
+// 16-column panel below and including the diagonal block is factored in registers, 32 rows per warp (lanes
+// 0-15 hold the diagonal block -- redundantly in every warp --, lanes 16-31 sixteen panel rows).  A pivot
+// step broadcasts the UNSCALED column by shuffles and updates with a_rj a_cj / d_j, so the dependent chain
+// per pivot is shuffle -> reciprocal -> two FMAs and needs no block barrier; columns are scaled by
+// 1/sqrt(d_j) after the 16 pivots.  The trailing rows are then updated on the FP64 tensor pipe.
+// Returns false if a pivot is not positive (it is then replaced by 1).
+__device__ __forceinline__ bool tile_potrf(double* __restrict__ S, double* __restrict__ rdiag, int tid) {
+  const int warp = tid >> 5, lane = tid & 31;
   bool ok = true;
-  for (int j = 0; j < CT; ++j) {
-    __syncthreads();
-    double d = S[j * TLD + j];
-    if (!(d > 0.0)) { ok = false; d = 1.0; }
-    const double inv = 1.0 / d;
+#pragma unroll 1
+  for (int b = 0; b < CT / 16; ++b) {
+    const int o = b * 16;
+    const int npanel = CT - o - 16;                        // rows below the diagonal block
+    const int nwarps = npanel > 0 ? npanel / 16 : 1;
+    if (warp < nwarps) {
+      const bool isdiag = lane < 16;
+      const int row = isdiag ? o + lane : o + 16 * (warp + 1) + (lane - 16);
+      const bool live = isdiag || npanel > 0;
+      double a[16], myd = 1.0;
+      const double* src = S + (live ? row : o) * TLD + o;
 #pragma unroll
-    for (int a = 0; a < 4; ++a) {
-      const int r = ty + 16 * a;
-      if (r > j) {
-        const double lr = S[r * TLD + j] * inv;
+      for (int c = 0; c < 16; c += 2) {
+        const double2 v = *reinterpret_cast<const double2*>(src + c);
+        a[c] = v.x; a[c + 1] = v.y;
+      }
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-          const int c = tx + 16 * b;
-          if (c > j && c <= r) S[r * TLD + c] = fma(-lr, S[c * TLD + j], S[r * TLD + c]);
+      for (int j = 0; j < 16; ++j) {
+        const double d = __shfl_sync(0xffffffffu, a[j], j);
+        double ac[16];
+#pragma unroll
+        for (int c = j + 1; c < 16; ++c) ac[c] = __shfl_sync(0xffffffffu, a[j], c);
+        // the positivity test stays off the dependent chain: a bad pivot poisons the tile, which is
+        // reported as HSP_ENOTPD by the caller
+        if (!(d > 0.0)) ok = false;
+        if (lane == j) myd = d;
+        const double r = fast_rcp(d);
+        if (j + 1 < 16) a[j + 1] = fma(-(a[j] * ac[j + 1]), r, a[j + 1]);   // next pivot first: one FMA after r
+        const double sc = a[j] * r;
+#pragma unroll
+        for (int c = j + 2; c < 16; ++c) a[c] = fma(-sc, ac[c], a[c]);
+      }
+      if (!(myd > 0.0)) myd = 1.0;
+      const double myrinv = rsqrt(myd);                    // lane j < 16: 1 / sqrt(d_j)
+      if (warp == 0 && isdiag) rdiag[o + lane] = myrinv;
+#pragma unroll
+      for (int j = 0; j < 16; ++j) a[j] *= __shfl_sync(0xffffffffu, myrinv, j);   // lane j: d_j / sqrt(d_j)
+      if (live && (warp == 0 || !isdiag)) {
+        double* dst = S + row * TLD + o;
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) {
+          double2 v;
+          v.x = (isdiag && c > lane) ? 0.0 : a[c];
+          v.y = (isdiag && c + 1 > lane) ? 0.0 : a[c + 1];
+          *reinterpret_cast<double2*>(dst + c) = v;
         }
       }
     }
-  }
-  __syncthreads();
-  if (tid < CT) {
-    double d = S[tid * TLD + tid];
-    if (!(d > 0.0)) d = 1.0;
-    dsq[tid] = 1.0 / sqrt(d);
-  }
-  __syncthreads();
-  double v[4][4];
+    __syncthreads();
+    if (npanel > 0) {
+      // trailing update: S[r][c] -= sum_{m<16} S[r][o+m] S[c][o+m] for o+16 <= c <= r < 64, 8x8 blocks
+      const int o2 = o + 16, nb8 = npanel / 8, g = lane >> 2, t = lane & 3;
+      const int nblocks = nb8 * (nb8 + 1) / 2;
+      for (int q0 = warp; q0 < nblocks; q0 += 3 * (kCholThreads / 32)) {
+        double c[3][2];
+        double* cp[3];
+        const double *ap[3], *bp[3];
+        bool on[3];
 #pragma unroll
-  for (int a = 0; a < 4; ++a)
+        for (int u = 0; u < 3; ++u) {
+          const int q = q0 + u * (kCholThreads / 32);
+          on[u] = q < nblocks;
+          int rb = 0, rem = on[u] ? q : 0;
+          while (rem >= rb + 1) { rem -= rb + 1; ++rb; }
+          const int cb = rem;
+          cp[u] = S + (o2 + rb * 8 + g) * TLD + o2 + cb * 8 + 2 * t;
+          ap[u] = S + (o2 + rb * 8 + g) * TLD + o + t;
+          bp[u] = S + (o2 + cb * 8 + g) * TLD + o + t;
+          const double2 c0 = *reinterpret_cast<const double2*>(cp[u]);
+          c[u][0] = c0.x; c[u][1] = c0.y;
+        }
 #pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      const int r = ty + 16 * a, c = tx + 16 * b;
-      double x = 0.0;
-      if (r > c) x = S[r * TLD + c] * dsq[c];
-      else if (r == c) { double d = S[r * TLD + r]; if (!(d > 0.0)) d = 1.0; x = d * dsq[r]; }
-      v[a][b] = x;
+        for (int kk = 0; kk < 16; kk += 4)
+#pragma unroll
+          for (int u = 0; u < 3; ++u) dmma(c[u], -ap[u][kk], bp[u][kk]);
+#pragma unroll
+        for (int u = 0; u < 3; ++u)
+          if (on[u]) *reinterpret_cast<double2*>(cp[u]) = make_double2(c[u][0], c[u][1]);
+      }
+      __syncthreads();
     }
-  __syncthreads();
-#pragma unroll
-  for (int a = 0; a < 4; ++a)
-#pragma unroll
-    for (int b = 0; b < 4; ++b) S[(ty + 16 * a) * TLD + tx + 16 * b] = v[a][b];
-  __syncthreads();
+  }
   return ok;
 }
 
+// C (H x H, stride TLD) = sgn * A B with A, B row-major H x H blocks (stride TLD) in shared memory, on the
+// FP64 tensor pipe; the H/8 x H/8 output blocks are dealt to `nw` warps, this warp being number `w`.
+template <int H>
+__device__ __forceinline__ void sub_mma(const double* __restrict__ A, const double* __restrict__ B, double* __restrict__ C,
+                                        bool neg, int w, int nw, int lane) {
+  const int g = lane >> 2, t = lane & 3;
+  constexpr int NB = H / 8;
+  for (int q = w; q < NB * NB; q += nw) {
+    const int mb = q / NB, nb = q % NB;
+    double c[2] = {0.0, 0.0};
+    const double* ap = A + (mb * 8 + g) * TLD + t;
+    const double* bp = B + t * TLD + nb * 8 + g;
+#pragma unroll
+    for (int kk = 0; kk < H; kk += 4) dmma(c, ap[kk], bp[kk * TLD]);
+    *reinterpret_cast<double2*>(C + (mb * 8 + g) * TLD + nb * 8 + 2 * t) = neg ? make_double2(-c[0], -c[1]) : make_double2(c[0], c[1]);
+  }
+}
+
 // X = S^-1 for the lower-triangular 64x64 tile S (stride TLD); X (stride TLD) gets the full tile
-// (zeros above the diagonal).  16x16 diagonal blocks by substitution (one thread per column, registers),
-// then two merge levels  [A 0; B C]^-1 = [A^-1 0; -C^-1 B A^-1  C^-1].
-__device__ __forceinline__ void tile_trinv(const double* __restrict__ S, const double* __restrict__ dsq,
+// (zeros above the diagonal).  16x16 diagonal blocks by column-oriented substitution (one thread per
+// column, registers), then two merge levels  [A 0; B C]^-1 = [A^-1 0; -C^-1 (B A^-1)  C^-1]  whose small
+// products run on the FP64 tensor pipe.  rdiag[r] = 1 / S[r][r].
+__device__ __forceinline__ void tile_trinv(const double* __restrict__ S, const double* __restrict__ rdiag,
                                            double* __restrict__ X, int tid) {
-  for (int e = tid; e < CT * TLD; e += kCholThreads) X[e] = 0.0;
+  const int warp = tid >> 5, lane = tid & 31;
+  for (int e = tid; e < CT * TLD / 2; e += kCholThreads) reinterpret_cast<double2*>(X)[e] = make_double2(0.0, 0.0);
   __syncthreads();
   if (tid < CT) {
     const int b0 = (tid >> 4) * 16, c = tid & 15;
     double x[16];
 #pragma unroll
-    for (int r = 0; r < 16; ++r) {
-      double s = (r == c) ? 1.0 : 0.0;
+    for (int r = 0; r < 16; ++r) x[r] = (r == c) ? 1.0 : 0.0;
 #pragma unroll
-      for (int m = 0; m < r; ++m) s = fma(-S[(b0 + r) * TLD + b0 + m], x[m], s);
-      x[r] = (r >= c) ? s * dsq[b0 + r] : 0.0;          // 1 / L_rr = 1 / sqrt(d_r)
+    for (int m = 0; m < 16; ++m) {
+      const double xm = x[m] * rdiag[b0 + m];
+      x[m] = xm;
+#pragma unroll
+      for (int r = m + 1; r < 16; ++r) x[r] = fma(-S[(b0 + r) * TLD + b0 + m], xm, x[r]);
     }
 #pragma unroll
     for (int r = 0; r < 16; ++r) X[(b0 + r) * TLD + b0 + c] = x[r];
   }
   __syncthreads();
-  for (int h = 16; h < CT; h <<= 1) {
-    const int nblk = CT / (2 * h);
-    // T = B A^-1 into the (zero) upper-right block of X
-    for (int e = tid; e < nblk * h * h; e += kCholThreads) {
-      const int blk = e / (h * h), r = (e / h) % h, c = e % h, off = blk * 2 * h;
-      double s = 0.0;
-      for (int m = c; m < h; ++m) s = fma(S[(off + h + r) * TLD + off + m], X[(off + m) * TLD + off + c], s);
-      X[(off + r) * TLD + off + h + c] = s;
+  {
+    // h = 16: the two 32x32 diagonal blocks, four warps each
+    const int off = (warp >> 2) * 32, w = warp & 3;
+    sub_mma<16>(S + (off + 16) * TLD + off, X + off * TLD + off, X + off * TLD + off + 16, false, w, 4, lane);      // T = B A^-1
+    __syncthreads();
+    sub_mma<16>(X + (off + 16) * TLD + off + 16, X + off * TLD + off + 16, X + (off + 16) * TLD + off, true, w, 4, lane);   // -C^-1 T
+    __syncthreads();
+    for (int e = tid; e < 2 * 16 * 16; e += kCholThreads) {
+      const int blk = e >> 8, r = (e >> 4) & 15, c = e & 15;
+      X[(blk * 32 + r) * TLD + blk * 32 + 16 + c] = 0.0;
     }
     __syncthreads();
-    // lower-left block = -C^-1 T
-    for (int e = tid; e < nblk * h * h; e += kCholThreads) {
-      const int blk = e / (h * h), r = (e / h) % h, c = e % h, off = blk * 2 * h;
-      double s = 0.0;
-      for (int m = 0; m <= r; ++m) s = fma(X[(off + h + r) * TLD + off + h + m], X[(off + m) * TLD + off + h + c], s);
-      X[(off + h + r) * TLD + off + c] = -s;
-    }
+  }
+  {
+    // h = 32
+    sub_mma<32>(S + 32 * TLD, X, X + 32, false, warp, 8, lane);
     __syncthreads();
-    for (int e = tid; e < nblk * h * h; e += kCholThreads) {
-      const int blk = e / (h * h), r = (e / h) % h, c = e % h, off = blk * 2 * h;
-      X[(off + r) * TLD + off + h + c] = 0.0;
-    }
+    sub_mma<32>(X + 32 * TLD + 32, X + 32, X + 32 * TLD, true, warp, 8, lane);
+    __syncthreads();
+    for (int e = tid; e < 32 * 32; e += kCholThreads) X[(e >> 5) * TLD + 32 + (e & 31)] = 0.0;
     __syncthreads();
   }
 }
 
 __global__ void __launch_bounds__(kCholThreads, 1)
-chol_dataflow_kernel(const double* __restrict__ G, const double* __restrict__ lam_inv2, Ctl* __restrict__ ctl,
-                     double* __restrict__ L, double* __restrict__ W, double* __restrict__ Wt, int* __restrict__ flags,
-                     int p, int nt) {
+chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_inv2, Ctl* __restrict__ ctl,
+                 double* __restrict__ L, double* __restrict__ W, double* __restrict__ Wt, double* __restrict__ ws,
+                 int* __restrict__ flags, const CholTask* __restrict__ tasks, const int* __restrict__ list_off, int p,
+                 int nt, unsigned long long* __restrict__ trace) {
   extern __shared__ __align__(16) double pool[];
-  double* dsq = pool + (size_t)NST * kStageDoubles;          // 64 doubles of scratch after the pool
+  double* S = pool + kPoolDoubles;                   // 64 x TLD
+  double* X = S + CT * TLD;                          // 64 x TLD
+  double* rdiag = X + CT * TLD;                      // 64
   const int P = nt * CT;
-  const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+  const int tid = threadIdx.x;
+  const Frag f(tid);
   int* fL = flags;
   int* fB = flags + (size_t)nt * nt;
+  int* fP = fB + (size_t)nt * nt;
   const double tau_inv2 = ctl->tau_inv2;
-  const long long ntasks = (long long)nt * nt;
 
-  for (long long t = blockIdx.x; t < ntasks; t += gridDim.x) {
-    const int j = (int)(t / nt), rr = (int)(t % nt);
-    const bool isL = rr < nt - j;
-    const int i = isL ? j + rr : rr - (nt - j);
-    // operands of the k loop: acc -= MA(ra,k) MB(rb,k)^T, k in [kbeg, kend)
+  const int t_end = list_off[blockIdx.x + 1];
+  for (int ti = list_off[blockIdx.x]; ti < t_end; ++ti) {
+    const CholTask tk = tasks[ti];
+    if (trace != nullptr && tid == 0) trace[4 * (size_t)ti] = globaltimer_ns();
+    const bool isL = tk.type == 0;
+    const int i = tk.i, j = tk.j;
+    // operands of the k loop: acc -= MA(ra,k) MB(rb,k)^T
     const double* MA = L;
     const double* MB = isL ? L : Wt;
     const int ra = isL ? i : j, rb = isL ? j : i;
-    const int kbeg = isL ? 0 : i, kend = j;
+    const int kbeg = tk.kbeg, kend = tk.kend;
 
-    double acc[4][4];
+    double acc[4][2][2];
+    if (tk.slot_in >= 0) {
+      wait_flag(&fP[tk.slot_in]);
+      const double2* src = reinterpret_cast<const double2*>(ws + (size_t)tk.slot_in * CT * CT);
 #pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        double v = 0.0;
-        if (isL) {                                   // c: Q tile, padded with the identity
-          const int gr = i * CT + ty + 16 * a, gc = j * CT + tx + 16 * b;
-          if (gr < p && gc < p) {
-            v = G[(size_t)gr * p + gc];
-            if (gr == gc) v = fma(tau_inv2, lam_inv2[gr], v);
-          } else if (gr == gc) v = 1.0;
-        }
-        acc[a][b] = v;
+      for (int q = 0; q < 8; ++q) {
+        const double2 v = __ldcg(src + q * kCholThreads + tid);
+        acc[q >> 1][q & 1][0] = v.x; acc[q >> 1][q & 1][1] = v.y;
       }
+    } else {
+#pragma unroll
+      for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+        for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            double v = 0.0;
+            if (isL) {                               // c: Q tile, padded with the identity
+              const int gr = i * CT + f.row0 + mb * 8 + f.g, gc = j * CT + f.col0 + nb * 8 + 2 * f.t + e;
+              if (gr < p && gc < p) {
+                v = G[(size_t)gr * p + gc];
+                if (gr == gc) v = fma(tau_inv2, lam_inv2[gr], v);
+              } else if (gr == gc) v = 1.0;
+            }
+            acc[mb][nb][e] = v;
+          }
+    }
 
     const int nchunks = (kend - kbeg) * (CT / KC);
     auto issue = [&](int c) {
@@ -242,7 +355,7 @@ chol_dataflow_kernel(const double* __restrict__ G, const double* __restrict__ la
         cp_async16(sb + row * CLD + pc * 2, gb + (size_t)row * P + pc * 2);
       }
     };
-    __syncthreads();                                 // the pool is free (previous task's finalize is over)
+    __syncthreads();                                 // the pool, S and X are free (previous task is over)
     for (int c = 0; c < NST - 1; ++c) {
       if (c < nchunks) issue(c);
       cp_async_commit();
@@ -253,28 +366,40 @@ chol_dataflow_kernel(const double* __restrict__ G, const double* __restrict__ la
       if (c + NST - 1 < nchunks) issue(c + NST - 1);
       cp_async_commit();
       const double* sa = pool + (size_t)(c % NST) * kStageDoubles;
-      tile_mac<CLD, CLD, KC, true>(sa, sa + CT * CLD, ty, tx, acc);
+      tile_mma<CLD, CLD, KC, true>(sa, sa + CT * CLD, f, acc);
     }
     cp_async_wait<0>();
-    __syncthreads();
+    if (trace != nullptr && tid == 0) trace[4 * (size_t)ti + 1] = globaltimer_ns();
 
-    double* S = pool;                                // 64 x TLD
-    double* X = pool + CT * TLD;                     // 64 x TLD
-    if (isL && i == j) {
+    if (tk.slot_out >= 0) {
+      // ---- prefix task: park the partial accumulator
+      double2* dst = reinterpret_cast<double2*>(ws + (size_t)tk.slot_out * CT * CT);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) __stcg(dst + q * kCholThreads + tid, make_double2(acc[q >> 1][q & 1][0], acc[q >> 1][q & 1][1]));
+      __threadfence();
+      __syncthreads();
+      if (tid == 0) st_release(&fP[tk.slot_out], 1);
+    } else if (isL && i == j) {
       // ---- diagonal: L_jj = chol(acc), W_jj = L_jj^-1
 #pragma unroll
-      for (int a = 0; a < 4; ++a)
+      for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
-        for (int b = 0; b < 4; ++b) S[(ty + 16 * a) * TLD + tx + 16 * b] = acc[a][b];
-      const bool ok = tile_potrf(S, dsq, tid, ty, tx);
+        for (int nb = 0; nb < 2; ++nb)
+          *reinterpret_cast<double2*>(S + (f.row0 + mb * 8 + f.g) * TLD + f.col0 + nb * 8 + 2 * f.t) =
+              make_double2(acc[mb][nb][0], acc[mb][nb][1]);
+      __syncthreads();
+      const bool ok = tile_potrf(S, rdiag, tid);
       if (!ok && tid == 0) atomicCAS(&ctl->status, 0, -4);
-      tile_trinv(S, dsq, X, tid);
-      for (int e = tid; e < CT * CT; e += kCholThreads) {
-        const int r = e / CT, c = e % CT;
+      tile_trinv(S, rdiag, X, tid);
+      for (int e = tid; e < CT * CT / 2; e += kCholThreads) {
+        const int r = e / (CT / 2), c = (e % (CT / 2)) * 2;
         const size_t g = (size_t)(j * CT + r) * P + j * CT + c;
-        L[g] = S[r * TLD + c];
-        W[g] = X[r * TLD + c];
-        Wt[g] = X[c * TLD + r];
+        double2 l = *reinterpret_cast<const double2*>(S + r * TLD + c);
+        if (c > r) l.x = 0.0;
+        if (c + 1 > r) l.y = 0.0;
+        *reinterpret_cast<double2*>(L + g) = l;
+        *reinterpret_cast<double2*>(W + g) = *reinterpret_cast<const double2*>(X + r * TLD + c);
+        *reinterpret_cast<double2*>(Wt + g) = make_double2(X[c * TLD + r], X[(c + 1) * TLD + r]);
       }
       __threadfence();
       __syncthreads();
@@ -288,47 +413,56 @@ chol_dataflow_kernel(const double* __restrict__ G, const double* __restrict__ la
         cp_async16(X + row * TLD + pc * 2, wjj + (size_t)row * P + pc * 2);
       }
       cp_async_commit();
-      double out[4][4];
+      double out[4][2][2];
 #pragma unroll
-      for (int a = 0; a < 4; ++a)
+      for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
-        for (int b = 0; b < 4; ++b) out[a][b] = 0.0;
+        for (int nb = 0; nb < 2; ++nb) out[mb][nb][0] = out[mb][nb][1] = 0.0;
       if (isL) {
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
+        for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
-          for (int b = 0; b < 4; ++b) S[(ty + 16 * a) * TLD + tx + 16 * b] = acc[a][b];
+          for (int nb = 0; nb < 2; ++nb)
+            *reinterpret_cast<double2*>(S + (f.row0 + mb * 8 + f.g) * TLD + f.col0 + nb * 8 + 2 * f.t) =
+                make_double2(acc[mb][nb][0], acc[mb][nb][1]);
         cp_async_wait<0>();
         __syncthreads();
-        tile_mac<TLD, TLD, CT, false>(S, X, ty, tx, out);          // L_ij = A W_jj^T
+        tile_mma<TLD, TLD, CT, false>(S, X, f, out);               // L_ij = A W_jj^T
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
+        for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
-          for (int b = 0; b < 4; ++b) L[(size_t)(i * CT + ty + 16 * a) * P + j * CT + tx + 16 * b] = out[a][b];
+          for (int nb = 0; nb < 2; ++nb)
+            *reinterpret_cast<double2*>(L + (size_t)(i * CT + f.row0 + mb * 8 + f.g) * P + j * CT + f.col0 + nb * 8 + 2 * f.t) =
+                make_double2(out[mb][nb][0], out[mb][nb][1]);
         __threadfence();
         __syncthreads();
         if (tid == 0) st_release(&fL[(size_t)i * nt + j], 1);
       } else {
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
+        for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
-          for (int b = 0; b < 4; ++b) S[(tx + 16 * b) * TLD + ty + 16 * a] = acc[a][b];   // transposed
+          for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+              S[(f.col0 + nb * 8 + 2 * f.t + e) * TLD + f.row0 + mb * 8 + f.g] = acc[mb][nb][e];   // transposed
         cp_async_wait<0>();
         __syncthreads();
-        tile_mac<TLD, TLD, CT, false>(X, S, ty, tx, out);          // W_ji = W_jj A
+        tile_mma<TLD, TLD, CT, false>(X, S, f, out);               // W_ji = W_jj A
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
+        for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
-          for (int b = 0; b < 4; ++b) {
-            const int r = j * CT + ty + 16 * a, c = i * CT + tx + 16 * b;
-            W[(size_t)r * P + c] = out[a][b];
-            Wt[(size_t)c * P + r] = out[a][b];
+          for (int nb = 0; nb < 2; ++nb) {
+            const int r = j * CT + f.row0 + mb * 8 + f.g, c = i * CT + f.col0 + nb * 8 + 2 * f.t;
+            *reinterpret_cast<double2*>(W + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
+            Wt[(size_t)c * P + r] = out[mb][nb][0];
+            Wt[(size_t)(c + 1) * P + r] = out[mb][nb][1];
           }
         __threadfence();
         __syncthreads();
         if (tid == 0) st_release(&fB[(size_t)i * nt + j], 1);
       }
     }
+    if (trace != nullptr && tid == 0) { trace[4 * (size_t)ti + 2] = globaltimer_ns(); trace[4 * (size_t)ti + 3] = blockIdx.x; }
   }
 }
 
@@ -386,45 +520,68 @@ static int env_int2(const char* name, int dflt) {
   return (v && *v) ? atoi(v) : dflt;
 }
 
-// Number of CTAs for the Cholesky branch.  When the branch is expected to hide behind the fused pass
-// it gets `k` SMs of its own and the fused pass the other num_sms - k; otherwise every SM.
-int chol_plan_ctas(int p, int num_sms, double fused_ms_estimate, bool* overlap) {
-  const int nt = chol_tiles(p);
-  const double flops = 2.0 * (double)p * p * p / 3.0;             // Cholesky + inverse factor
-  const double per_sm = 0.5 * 2.0 * 64.0 * 1.9e9;                 // ~50 % of 64 DFMA/clk/SM
-  int k = env_int2("HSP_CHOL_CTAS", 0);
-  bool ov;
-  if (k > 0) {
-    ov = k < num_sms;
+// Build the static schedule and decide how many SMs the Cholesky branch gets.  When the cost model says the
+// branch hides behind the fused pass on K SMs of its own (the pass keeps num_sms - K), the smallest such K
+// is taken; otherwise the branch uses every SM and runs before/after the pass.
+cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_estimate) {
+  pl->p = p; pl->nt = chol_tiles(p); pl->P = chol_ld(p);
+  const int nt = pl->nt;
+  const long long tile_tasks = (long long)nt * nt;
+  CholSchedule best;
+  int k_env = env_int2("HSP_CHOL_CTAS", 0);
+  if (k_env > num_sms) k_env = num_sms;
+  if (k_env > 0) {
+    best = chol_build_schedule(nt, nt, (int)std::min<long long>(k_env, tile_tasks));
+    pl->overlap = k_env < num_sms;
   } else {
-    // measured on B200 (profiles/r01_b): the left-looking task chain costs ~35 us per tile column, and the
-    // kernel takes ~2.6x the time the flop count at 50 % of the DFMA rate suggests
-    const double critical_ms = nt * 0.035;
-    k = 8;
-    while (k < 48 && 2.6 * (flops / (k * per_sm)) * 1e3 > 0.85 * fused_ms_estimate) k += 4;
-    const double t = 2.6 * (flops / (k * per_sm)) * 1e3;
-    ov = t <= 0.9 * fused_ms_estimate && critical_ms <= 0.9 * fused_ms_estimate;
-    if (!ov) k = num_sms;
+    const double budget_us = 0.85 * fused_ms_estimate * 1e3;
+    const int cands[] = {2, 4, 6, 8, 10, 12, 16, 20, 24, 32, 40, 48};
+    bool found = false;
+    if (nt <= 40)
+      for (int k : cands) {
+        if (k > tile_tasks || k >= num_sms / 2) break;
+        CholSchedule s = chol_build_schedule(nt, nt, k);
+        if (s.makespan_us <= budget_us) { best = std::move(s); found = true; break; }
+      }
+    pl->overlap = found;
+    if (!found) best = chol_build_schedule(nt, nt, (int)std::min<long long>(num_sms, tile_tasks));
   }
-  const long long ntasks = (long long)nt * nt;
-  if (k > ntasks) k = (int)ntasks;
-  if (k > num_sms) k = num_sms;
-  if (overlap) *overlap = ov;
-  return k;
+  pl->K = best.K; pl->n_slots = best.n_slots; pl->n_tasks = (int)best.tasks.size(); pl->est_us = best.makespan_us;
+  pl->n_flags = 2 * (size_t)nt * nt + (size_t)std::max(1, best.n_slots);
+  cudaError_t e = cudaMalloc(&pl->d_tasks, best.tasks.size() * sizeof(CholTask));
+  if (e == cudaSuccess) e = cudaMalloc(&pl->d_list_off, best.list_off.size() * sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc(&pl->d_flags, pl->n_flags * sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc(&pl->d_ws, (size_t)std::max(1, best.n_slots) * CT * CT * sizeof(double));
+  if (e == cudaSuccess) e = cudaMemcpy(pl->d_tasks, best.tasks.data(), best.tasks.size() * sizeof(CholTask), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(pl->d_list_off, best.list_off.data(), best.list_off.size() * sizeof(int), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess && env_int2("HSP_CHOL_TRACE", 0)) {
+    e = cudaMalloc(&pl->d_trace, best.tasks.size() * 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(pl->d_trace, 0, best.tasks.size() * 4 * sizeof(unsigned long long));
+  }
+  pl->h_tasks = best.tasks;
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(chol_task_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCholSmem);
+  return e;
 }
 
-cudaError_t chol_prepare() {
-  return cudaFuncSetAttribute(chol_dataflow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCholSmem);
+void chol_plan_destroy(CholPlan* pl) {
+  if (pl->d_tasks) cudaFree(pl->d_tasks);
+  if (pl->d_list_off) cudaFree(pl->d_list_off);
+  if (pl->d_flags) cudaFree(pl->d_flags);
+  if (pl->d_ws) cudaFree(pl->d_ws);
+  if (pl->d_trace) cudaFree(pl->d_trace);
+  *pl = CholPlan{};
 }
 
-cudaError_t cholesky_launch(const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W, double* Wt,
-                            int* flags, int p, int ctas, cudaStream_t st, long long* launches) {
-  int nt = chol_tiles(p);
-  cudaError_t e = cudaMemsetAsync(flags, 0, chol_flag_count(p) * sizeof(int), st);
+cudaError_t cholesky_launch(const CholPlan& pl, const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W,
+                            double* Wt, cudaStream_t st, long long* launches) {
+  cudaError_t e = cudaMemsetAsync(pl.d_flags, 0, pl.n_flags * sizeof(int), st);
   if (e != cudaSuccess) return e;
-  void* args[] = {(void*)&G, (void*)&lam_inv2, (void*)&ctl, (void*)&L, (void*)&W, (void*)&Wt, (void*)&flags, (void*)&p,
-                  (void*)&nt};
-  e = cudaLaunchCooperativeKernel((const void*)chol_dataflow_kernel, dim3(ctas), dim3(kCholThreads), args, kCholSmem, st);
+  int p = pl.p, nt = pl.nt;
+  double* ws = pl.d_ws; int* flags = pl.d_flags; const CholTask* tasks = pl.d_tasks; const int* list_off = pl.d_list_off;
+  unsigned long long* trace = pl.d_trace;
+  void* args[] = {(void*)&G, (void*)&lam_inv2, (void*)&ctl, (void*)&L, (void*)&W, (void*)&Wt, (void*)&ws, (void*)&flags,
+                  (void*)&tasks, (void*)&list_off, (void*)&p, (void*)&nt, (void*)&trace};
+  e = cudaLaunchCooperativeKernel((const void*)chol_task_kernel, dim3(pl.K), dim3(kCholThreads), args, kCholSmem, st);
   if (launches) ++*launches;
   return e;
 }

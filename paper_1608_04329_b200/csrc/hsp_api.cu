@@ -37,7 +37,7 @@ struct hsp_state {
   void* own_X = nullptr; unsigned char* own_y = nullptr;
   double *G = nullptr, *L = nullptr, *W = nullptr, *Wt = nullptr, *beta = nullptr, *lam_inv2 = nullptr,
          *nu_inv = nullptr, *g = nullptr, *tv = nullptr, *partial = nullptr, *z = nullptr;
-  int* chol_flags = nullptr; int chol_ctas = 0; bool chol_overlap = false;
+  CholPlan chol{};
   signed char* side = nullptr;
   Ctl* ctl = nullptr;
   double *h_beta = nullptr, *h_lambda = nullptr, *h_tau = nullptr;
@@ -60,8 +60,9 @@ static void free_state(hsp_state* s) {
   if (s->stream2) cudaStreamDestroy(s->stream2);
   if (s->own_stream) cudaStreamDestroy(s->own_stream);
   void* ptrs[] = {s->own_X, s->own_y, s->G, s->L, s->W, s->Wt, s->beta, s->lam_inv2, s->nu_inv, s->g, s->tv, s->partial,
-                  s->z, s->side, s->chol_flags, s->ctl, s->h_beta, s->h_lambda, s->h_tau};
+                  s->z, s->side, s->ctl, s->h_beta, s->h_lambda, s->h_tau};
   for (void* q : ptrs) if (q) cudaFree(q);
+  chol_plan_destroy(&s->chol);
   delete s;
 }
 
@@ -102,7 +103,7 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
   }
   if (do_scales) { CK(scales_pre_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, B)); *kernels += 1; }
   if (do_beta) {
-    CK(cholesky_launch(s->G, s->lam_inv2, s->ctl, s->L, s->W, s->Wt, s->chol_flags, s->p, s->chol_ctas, B, kernels));
+    CK(cholesky_launch(s->chol, s->G, s->lam_inv2, s->ctl, s->L, s->W, s->Wt, B, kernels));
   }
   if (!serial && side_work) {
     CK(cudaEventRecord(s->ev_join, B));
@@ -148,16 +149,14 @@ static int create_common(hsp_state** out, hsp_state* s) {
   // its own and the pass the rest; otherwise both use every SM and run one after the other.
   const double x_bytes = (double)N * p * (s->dtype == HSP_F32 ? 4.0 : 8.0);
   const double fused_ms_est = x_bytes / 6.0e9 + 0.01;
-  s->chol_ctas = chol_plan_ctas(p, s->num_sms, fused_ms_est, &s->chol_overlap);
-  const int fused_sms = s->chol_overlap ? s->num_sms - s->chol_ctas : s->num_sms;
+  CK(chol_plan_create(&s->chol, p, s->num_sms, fused_ms_est));
+  const int fused_sms = s->chol.overlap ? s->num_sms - s->chol.K : s->num_sms;
   s->plan = fused_plan(s->dtype, N, p, fused_sms, s->X);
   // set opt-in shared-memory attributes now, outside any stream capture
   CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, -1, p, 0, nullptr, nullptr, nullptr, nullptr, s->stream));
-  CK(chol_prepare());
   const size_t pp = (size_t)p * p * sizeof(double), pv = (size_t)p * sizeof(double);
   const size_t P = (size_t)chol_ld(p), PP = P * P * sizeof(double), Pv = P * sizeof(double);
   CK(cudaMalloc(&s->G, pp)); CK(cudaMalloc(&s->L, PP)); CK(cudaMalloc(&s->W, PP)); CK(cudaMalloc(&s->Wt, PP));
-  CK(cudaMalloc(&s->chol_flags, chol_flag_count(p) * sizeof(int)));
   CK(cudaMalloc(&s->beta, pv)); CK(cudaMalloc(&s->lam_inv2, pv)); CK(cudaMalloc(&s->nu_inv, pv));
   CK(cudaMalloc(&s->g, Pv)); CK(cudaMalloc(&s->tv, Pv));     // padded to P with zeros (the GEMVs read whole tiles)
   CK(cudaMalloc(&s->partial, (size_t)s->plan.grid * s->plan.groups * pv));
@@ -426,8 +425,36 @@ int hsp_get_fused_pass_ms(hsp_state* s, double* ms, long long* launches) {
   return HSP_OK;
 }
 
+int hsp_get_plan(const hsp_state* s, int* fused_ctas, int* chol_ctas, int* overlap, double* chol_est_us) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  if (fused_ctas) *fused_ctas = s->plan.grid;
+  if (chol_ctas) *chol_ctas = s->chol.K;
+  if (overlap) *overlap = s->chol.overlap ? 1 : 0;
+  if (chol_est_us) *chol_est_us = s->chol.est_us;
+  return HSP_OK;
+}
 long long hsp_get_launch_count(const hsp_state* s) { return s ? s->launches : 0; }
 const char* hsp_fused_variant(const hsp_state* s) { return (s && s->plan.variant == 1) ? "tma" : "generic"; }
+
+long long hsp_dbg_chol_trace(const hsp_state* s, long long* rows, long long capacity) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  const CholPlan& pl = s->chol;
+  const long long n = (long long)pl.h_tasks.size();
+  if (!rows) return n;
+  if (capacity < n) return fail(HSP_EINVAL, "capacity is smaller than the number of tasks");
+  CK(cudaStreamSynchronize(s->stream));
+  std::vector<unsigned long long> tr((size_t)n * 4, 0ull);
+  if (pl.d_trace) CK(cudaMemcpy(tr.data(), pl.d_trace, tr.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  std::vector<int> cta_of((size_t)n, 0);
+  for (long long q = 0; q < n; ++q) {
+    const CholTask& t = pl.h_tasks[(size_t)q];
+    long long* r = rows + 12 * q;
+    r[0] = t.type; r[1] = t.i; r[2] = t.j; r[3] = t.kbeg; r[4] = t.kend; r[5] = t.slot_in; r[6] = t.slot_out;
+    r[7] = (long long)tr[4 * q + 3]; r[8] = (long long)tr[4 * q]; r[9] = (long long)tr[4 * q + 1]; r[10] = (long long)tr[4 * q + 2];
+    r[11] = 0;
+  }
+  return n;
+}
 
 // ---- device unit-test hooks ----------------------------------------------------------------------
 __global__ void dbg_philox_kernel(const unsigned* ctr, const unsigned* key, unsigned* out, long long n) {

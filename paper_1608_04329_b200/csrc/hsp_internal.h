@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
+#include <vector>
 
 namespace hsp {
 
@@ -44,14 +45,38 @@ cudaError_t gram_launch(const void* X, int dtype, long long N, int p, double* G,
                         cudaStream_t st);
 int gram_splits(long long N, int p, int num_sms);
 
-// ---- Q build (c), Cholesky + inverse factor (d1), beta draw (d2): cholesky.cu
+// ---- Q build (c), Cholesky + inverse factor (d1), beta draw (d2): cholesky.cu, chol_schedule.cu
+// One tile task of the Cholesky task graph (64x64 tiles).  type 0: tile L(i,j), i >= j; type 1: inverse tile
+// W(j,i), i < j.  The task accumulates k in [kbeg, kend); slot_in >= 0: start from the partial accumulator in
+// that workspace slot (else from the Q tile / zero); slot_out >= 0: store the partial accumulator there
+// instead of finalising the tile.
+struct CholTask { int type, i, j, kbeg, kend, slot_in, slot_out, pad; };
+struct CholSchedule {
+  int K = 0, n_slots = 0;
+  double makespan_us = 0.0;          // cost-model estimate
+  std::vector<CholTask> tasks;       // concatenated per-CTA lists
+  std::vector<int> list_off;         // K + 1 offsets into tasks
+};
+CholSchedule chol_build_schedule(int nt, int sb_tiles, int K);
+
+struct CholPlan {
+  int p = 0, nt = 0, P = 0, K = 0, n_slots = 0, n_tasks = 0;
+  bool overlap = false;              // the branch is expected to hide behind the fused pass on K SMs of its own
+  double est_us = 0.0;
+  CholTask* d_tasks = nullptr;
+  int* d_list_off = nullptr;
+  int* d_flags = nullptr;            // [nt*nt] L tiles, [nt*nt] inverse tiles, [n_slots] partials
+  size_t n_flags = 0;
+  double* d_ws = nullptr;            // n_slots x 4096 doubles
+  unsigned long long* d_trace = nullptr;   // HSP_CHOL_TRACE=1: per task {start, k-loop end, end} ns and the CTA
+  std::vector<CholTask> h_tasks;     // host copy of the schedule (for hsp_dbg_chol_trace)
+};
 int chol_tiles(int p);                 // nt = ceil(p / 64)
 int chol_ld(int p);                    // P = 64 nt: leading dimension of L, W, Wt (padded with the identity)
-size_t chol_flag_count(int p);         // ints of per-tile "done" flags
-int chol_plan_ctas(int p, int num_sms, double fused_ms_estimate, bool* overlap);
-cudaError_t chol_prepare();
-cudaError_t cholesky_launch(const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W, double* Wt,
-                            int* flags, int p, int ctas, cudaStream_t st, long long* launches);
+cudaError_t chol_plan_create(CholPlan* plan, int p, int num_sms, double fused_ms_estimate);
+void chol_plan_destroy(CholPlan* plan);
+cudaError_t cholesky_launch(const CholPlan& plan, const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W,
+                            double* Wt, cudaStream_t st, long long* launches);
 cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g, double* tv, double* beta, int p,
                               unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches);
 
