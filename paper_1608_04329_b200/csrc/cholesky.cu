@@ -466,53 +466,116 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
   }
 }
 
-// d2, first half: t = W g + e (L t = g + L e), one warp per row; e_j = Phi^-1(U_A(j, k, E)).
-constexpr int kGemvWarps = 8;
-__global__ void __launch_bounds__(kGemvWarps * 32)
-beta_gemv1_kernel(const double* __restrict__ W, const double* __restrict__ g, double* __restrict__ tv, int p, int P,
-                  unsigned long long seed, const Ctl* __restrict__ ctl) {
-  const int row = blockIdx.x * kGemvWarps + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-  if (row >= p) return;
-  const double* w = W + (size_t)row * P;
-  const int end = (row / CT + 1) * CT;               // W is zero right of the diagonal inside its tile
-  double s0 = 0.0, s1 = 0.0;
-  for (int c = 2 * lane; c < end; c += 64) {
-    const double2 a = *reinterpret_cast<const double2*>(w + c);
-    const double2 b = *reinterpret_cast<const double2*>(g + c);
-    s0 = fma(a.x, b.x, s0);
-    s1 = fma(a.y, b.y, s1);
-  }
-  double s = s0 + s1;
+// ---- d2: beta = Q^-1 g + L^-T e as two triangular matrix-vector products with the inverse factor,
+//   t = W g + e  (L t = g + L e)   and   beta = Wt t  (L^T beta = t),   e_j = Phi^-1(U_A(j, k, E)).
+// One warp per row; a lane keeps up to 16 double2 of its row in flight (one pass covers 1024 columns).
+// Both kernels are launched with programmatic stream serialisation: the first pass over the row of W / Wt
+// (ready since the Cholesky branch joined) and the normal variate are issued BEFORE griddepcontrol.wait,
+// i.e. while the preceding kernel (reduce / first product) is still running.
+constexpr int kGemvWarps = 4;
+constexpr int kGemvPass = 1024;                      // columns per pass: 32 lanes x 16 double2
+
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+__device__ __forceinline__ void gemv_load(double2 (&w)[16], const double* __restrict__ row, int base, int lo, int hi, int lane) {
 #pragma unroll
-  for (int off = 16; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
-  if (lane == 0) {
-    const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
-    tv[row] = s + norm_inv(uniform_a(seed, (unsigned long long)row, sweep, TAG_E));
+  for (int i = 0; i < 16; ++i) {
+    const int c = base + 2 * (lane + 32 * i);
+    w[i] = (c >= lo && c < hi) ? __ldcg(reinterpret_cast<const double2*>(row + c)) : make_double2(0.0, 0.0);
+  }
+}
+// x is written by the preceding kernel and read after griddepcontrol.wait: it must NOT be a const __restrict__
+// (invariant, ld.global.nc) load, which the compiler may hoist above the wait; __ldcg is an ordinary L2 load.
+__device__ __forceinline__ void gemv_dot(const double2 (&w)[16], const double* x, int base, int lo, int hi, int lane,
+                                         double& s0, double& s1) {
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const int c = base + 2 * (lane + 32 * i);
+    if (c >= lo && c < hi) {
+      const double2 b = __ldcg(reinterpret_cast<const double2*>(x + c));
+      s0 = fma(w[i].x, b.x, s0);
+      s1 = fma(w[i].y, b.y, s1);
+    }
   }
 }
 
-// d2, second half: beta = Wt t (L^T beta = t), one warp per row.
 __global__ void __launch_bounds__(kGemvWarps * 32)
-beta_gemv2_kernel(const double* __restrict__ Wt, const double* __restrict__ tv, double* __restrict__ beta, int p, int P,
-                  Ctl* __restrict__ ctl) {
+beta_gemv1_kernel(const double* __restrict__ W, const double* g, double* __restrict__ tv, int p, int P,
+                  unsigned long long seed, const Ctl* __restrict__ ctl) {
+  pdl_trigger();
   const int row = blockIdx.x * kGemvWarps + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-  if (row >= p) return;
-  const double* w = Wt + (size_t)row * P;
-  const int begin = (row / CT) * CT;                 // Wt is zero left of the diagonal inside its tile
+  const bool live = row < p;
+  const double* w = W + (size_t)(live ? row : 0) * P;
+  const int hi = live ? (row / CT + 1) * CT : 0;     // W is zero right of the diagonal inside its tile
+  double2 wr[16];
+  gemv_load(wr, w, 0, 0, hi, lane);
+  double e = 0.0;
+  if (lane == 0 && live) {
+    const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);   // written by the previous sweep's last kernel: complete
+    e = norm_inv(uniform_a(seed, (unsigned long long)row, sweep, TAG_E));
+  }
+  pdl_wait();                                        // g (reduce_partials_kernel) is complete and visible
   double s0 = 0.0, s1 = 0.0;
-  for (int c = begin + 2 * lane; c < P; c += 64) {
-    const double2 a = *reinterpret_cast<const double2*>(w + c);
-    const double2 b = *reinterpret_cast<const double2*>(tv + c);
-    s0 = fma(a.x, b.x, s0);
-    s1 = fma(a.y, b.y, s1);
+  gemv_dot(wr, g, 0, 0, hi, lane, s0, s1);
+  for (int base = kGemvPass; base < hi; base += kGemvPass) {
+    gemv_load(wr, w, base, 0, hi, lane);
+    gemv_dot(wr, g, base, 0, hi, lane, s0, s1);
   }
   double s = s0 + s1;
 #pragma unroll
   for (int off = 16; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
-  if (lane == 0) {
+  if (lane == 0 && live) tv[row] = s + e;
+}
+
+// Second product; also appends beta to the device history (row g of the hot-path table) and,
+// in the last CTA to finish, advances the sweep counter k <- k + 1.
+__global__ void __launch_bounds__(kGemvWarps * 32)
+beta_gemv2_kernel(const double* __restrict__ Wt, const double* tv, double* __restrict__ beta, int p, int P,
+                  Ctl* __restrict__ ctl) {
+  pdl_trigger();
+  const int row = blockIdx.x * kGemvWarps + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  const bool live = row < p;
+  const double* w = Wt + (size_t)(live ? row : 0) * P;
+  const int lo = (row / CT) * CT, hi = live ? P : 0; // Wt is zero left of the diagonal inside its tile
+  const int base0 = (lo / kGemvPass) * kGemvPass;
+  double2 wr[16];
+  gemv_load(wr, w, base0, lo, hi, lane);
+  const unsigned long long k = ctl->sweep + 1ull;
+  double* __restrict__ h_beta = ctl->h_beta;
+  const unsigned long long hrow = k - 1ull - ctl->hist_base;
+  pdl_wait();                                        // tv (beta_gemv1_kernel) is complete and visible
+  double s0 = 0.0, s1 = 0.0;
+  gemv_dot(wr, tv, base0, lo, hi, lane, s0, s1);
+  for (int base = base0 + kGemvPass; base < hi; base += kGemvPass) {
+    gemv_load(wr, w, base, lo, hi, lane);
+    gemv_dot(wr, tv, base, lo, hi, lane, s0, s1);
+  }
+  double s = s0 + s1;
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  if (lane == 0 && live) {
     beta[row] = s;
+    if (h_beta != nullptr) h_beta[hrow * (unsigned long long)p + row] = s;
     if (!isfinite(s)) atomicCAS(&ctl->status, 0, -5);
   }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    if (atomicAdd(&ctl->done, 1) == (int)gridDim.x - 1) { ctl->done = 0; ctl->sweep = k; }
+  }
+}
+
+// FREEZE_BETA (tests): beta stays; append it to the history and advance the sweep counter.
+__global__ void __launch_bounds__(256)
+beta_keep_kernel(const double* __restrict__ beta, int p, Ctl* __restrict__ ctl) {
+  const unsigned long long k = ctl->sweep + 1ull;
+  double* __restrict__ h_beta = ctl->h_beta;
+  const unsigned long long hrow = k - 1ull - ctl->hist_base;
+  if (h_beta != nullptr)
+    for (int j = threadIdx.x; j < p; j += blockDim.x) h_beta[hrow * (unsigned long long)p + j] = beta[j];
+  __syncthreads();
+  if (threadIdx.x == 0) ctl->sweep = k;
 }
 
 static int env_int2(const char* name, int dflt) {
@@ -586,13 +649,31 @@ cudaError_t cholesky_launch(const CholPlan& pl, const double* G, const double* l
   return e;
 }
 
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kern)(KArgs...), int grid, int block, cudaStream_t st, bool pdl, Args... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
 cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g, double* tv, double* beta, int p,
                               unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches) {
   const int P = chol_ld(p);
   const int grid = (p + kGemvWarps - 1) / kGemvWarps;
-  beta_gemv1_kernel<<<grid, kGemvWarps * 32, 0, st>>>(W, g, tv, p, P, seed, ctl);
-  beta_gemv2_kernel<<<grid, kGemvWarps * 32, 0, st>>>(Wt, tv, beta, p, P, ctl);
+  static const bool pdl = env_int2("HSP_NO_PDL", 0) == 0;
+  cudaError_t e = launch_pdl(beta_gemv1_kernel, grid, kGemvWarps * 32, st, pdl, W, g, tv, p, P, seed, (const Ctl*)ctl);
+  if (e != cudaSuccess) return e;
+  e = launch_pdl(beta_gemv2_kernel, grid, kGemvWarps * 32, st, pdl, Wt, (const double*)tv, beta, p, P, ctl);
   if (launches) *launches += 2;
+  return e;
+}
+
+cudaError_t beta_keep_launch(const double* beta, int p, Ctl* ctl, cudaStream_t st) {
+  beta_keep_kernel<<<1, 256, 0, st>>>(beta, p, ctl);
   return cudaGetLastError();
 }
 

@@ -77,17 +77,25 @@ static int drain_fused_events(hsp_state* s) {
 }
 
 // Enqueue one sweep.  `timed`: bracket the fused pass with CUDA events (direct-launch mode only).
+//   stream A:  fused pass (a1-a3) ------------------------------> [join] reduce (b) -> d2 (two products; k <- k+1)
+//   stream B:  scales (e1, e2, e3; lambda, tau history) -> Q build + Cholesky + inverse factor (c, d1)
 static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
   cudaStream_t A = s->stream;
   const bool serial = (s->flags & HSP_SERIAL) != 0;
   cudaStream_t B = serial ? A : s->stream2;
   const bool do_z = !(s->flags & HSP_FREEZE_Z), do_scales = !(s->flags & HSP_FREEZE_SCALES),
              do_beta = !(s->flags & HSP_FREEZE_BETA);
-  const bool side_work = do_scales || do_beta;
-  if (!serial && side_work) {
+  if (!serial) {
     CK(cudaEventRecord(s->ev_fork, A));
     CK(cudaStreamWaitEvent(B, s->ev_fork, 0));
   }
+  auto side_branch = [&]() -> int {
+    CK(scales_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, do_scales ? 0 : 1, B));
+    *kernels += 1;
+    if (do_beta) CK(cholesky_launch(s->chol, s->G, s->lam_inv2, s->ctl, s->L, s->W, s->Wt, B, kernels));
+    return HSP_OK;
+  };
+  if (serial) { const int rc = side_branch(); if (rc) return rc; }
   if (do_z) {
     if (timed) {
       if (s->tev_used + 2 > s->tev.size()) {
@@ -98,20 +106,16 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
     CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, s->N, s->p, s->seed, s->beta, s->ctl, s->partial,
                          (s->flags & HSP_STORE_Z) ? s->z : nullptr, A));
     if (timed) { CK(cudaEventRecord(s->tev[s->tev_used + 1], A)); s->tev_used += 2; }
-    CK(reduce_partials_launch(s->partial, s->plan.grid * s->plan.groups, s->p, s->g, A));
-    *kernels += 2;
+    *kernels += 1;
   }
-  if (do_scales) { CK(scales_pre_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, B)); *kernels += 1; }
-  if (do_beta) {
-    CK(cholesky_launch(s->chol, s->G, s->lam_inv2, s->ctl, s->L, s->W, s->Wt, B, kernels));
-  }
-  if (!serial && side_work) {
+  if (!serial) {
+    const int rc = side_branch(); if (rc) return rc;
     CK(cudaEventRecord(s->ev_join, B));
-    CK(cudaStreamWaitEvent(A, s->ev_join, 0));
+    CK(cudaStreamWaitEvent(A, s->ev_join, 0));      // before the reduce: the tail kernels then chain by PDL
   }
+  if (do_z) { CK(reduce_partials_launch(s->partial, s->plan.grid * s->plan.groups, s->p, s->g, A)); *kernels += 1; }
   if (do_beta) CK(beta_solve_launch(s->W, s->Wt, s->g, s->tv, s->beta, s->p, s->seed, s->ctl, A, kernels));
-  CK(scales_post_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, do_scales ? 0 : 1, A));
-  *kernels += 1;
+  else { CK(beta_keep_launch(s->beta, s->p, s->ctl, A)); *kernels += 1; }
   return HSP_OK;
 }
 
@@ -148,7 +152,7 @@ static int create_common(hsp_state** out, hsp_state* s) {
   // SM budget: when the Cholesky branch (c, d1) can hide behind the fused pass it gets chol_ctas SMs of
   // its own and the pass the rest; otherwise both use every SM and run one after the other.
   const double x_bytes = (double)N * p * (s->dtype == HSP_F32 ? 4.0 : 8.0);
-  const double fused_ms_est = x_bytes / 6.0e9 + 0.01;
+  const double fused_ms_est = x_bytes / 7.0e9 + 0.01;   // the pass streams X at ~7.2 TB/s on B200 (profiles/)
   CK(chol_plan_create(&s->chol, p, s->num_sms, fused_ms_est));
   const int fused_sms = s->chol.overlap ? s->num_sms - s->chol.K : s->num_sms;
   s->plan = fused_plan(s->dtype, N, p, fused_sms, s->X);
@@ -180,7 +184,7 @@ static int create_common(hsp_state** out, hsp_state* s) {
   CK(cudaMemsetAsync(s->L, 0, PP, s->stream));
   CK(cudaMemcpyAsync(s->lam_inv2, ones.data(), pv, cudaMemcpyHostToDevice, s->stream));
   CK(cudaMemcpyAsync(s->nu_inv, ones.data(), pv, cudaMemcpyHostToDevice, s->stream));
-  Ctl c{}; c.sweep = 0; c.hist_base = 0; c.tau_inv2 = 1.0; c.xi_inv = 1.0; c.status = 0;
+  Ctl c{}; c.sweep = 0; c.hist_base = 0; c.tau_inv2 = 1.0; c.xi_inv = 1.0; c.status = 0; c.done = 0;
   c.h_beta = c.h_lambda = c.h_tau = nullptr;
   CK(cudaMemcpyAsync(s->ctl, &c, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
   CK(cudaStreamSynchronize(s->stream));   // `ones` and `c` are stack/heap temporaries

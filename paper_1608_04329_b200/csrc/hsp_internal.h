@@ -13,7 +13,7 @@ struct Ctl {
   double tau_inv2;               // tau^-2
   double xi_inv;                 // xi^-1
   int status;                    // 0, or HSP_ENOTPD / HSP_ENUMERIC (first error wins)
-  int pad;
+  int done;                      // CTAs of beta_gemv2_kernel that have finished (the last one advances `sweep`)
   double* h_beta;                // device history of the current hsp_sweep call (may be null)
   double* h_lambda;
   double* h_tau;
@@ -30,6 +30,7 @@ struct FusedPlan {
   int lag;            // D
   int chunks;         // C
   int groups;         // G: row groups of compute warps (partial rows = grid * G)
+  int eta_mode;       // EM: arithmetic of the eta phase for fp32 X (fused_pass.cu)
   long long n_tiles;
 };
 
@@ -79,12 +80,11 @@ cudaError_t cholesky_launch(const CholPlan& plan, const double* G, const double*
                             double* Wt, cudaStream_t st, long long* launches);
 cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g, double* tv, double* beta, int p,
                               unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches);
+cudaError_t beta_keep_launch(const double* beta, int p, Ctl* ctl, cudaStream_t st);
 
 // ---- scale conditionals (e1, e2, e3) and draw output (g): scales.cu
-cudaError_t scales_pre_launch(const double* beta, double* lam_inv2, const double* nu_inv, Ctl* ctl, int p,
-                              unsigned long long seed, cudaStream_t st);
-cudaError_t scales_post_launch(const double* beta, const double* lam_inv2, double* nu_inv, Ctl* ctl, int p,
-                               unsigned long long seed, int freeze_scales, cudaStream_t st);
+cudaError_t scales_launch(const double* beta, double* lam_inv2, double* nu_inv, Ctl* ctl, int p, unsigned long long seed,
+                          int freeze_scales, cudaStream_t st);
 cudaError_t validate_y_launch(const unsigned char* y, long long N, int* bad, cudaStream_t st);
 cudaError_t side_launch(const unsigned char* y, long long N, signed char* side, cudaStream_t st);
 

@@ -1,7 +1,7 @@
 // scales.cu -- rows e1, e2, e3 and g of the hot-path table: the horseshoe scale conditionals of
 // eq. (12) exactly as PAPER.md:174-184 states them (with reading R1: tau^-2 is Gamma), by the
 // inversion -ln(u)/rate and Cheng's gamma sampler, plus the
-// append of (beta, lambda, tau) to the device history.
+// append of (lambda, tau) to the device history (beta is appended by beta_gemv2_kernel).
 #include <cuda_runtime.h>
 #include <cstdint>
 #include "hsp_device.cuh"
@@ -11,80 +11,60 @@ namespace hsp {
 
 constexpr int kScaleThreads = 1024;
 
-// e1 then e2 ("z and lambda^-2 in parallel, followed by tau^-2"); both use the OLD beta.
+// e1, e2 ("z and lambda^-2 in parallel, followed by tau^-2"; both use the OLD beta), then e3
+// (nu^-1 and xi^-1 "in parallel" with beta: they depend on the NEW lambda^-2, tau^-2 only, not
+// on beta, so they are drawn here, off the critical path), then row g for lambda and tau.  One CTA.
 __global__ void __launch_bounds__(kScaleThreads)
-scales_pre_kernel(const double* __restrict__ beta, double* __restrict__ lam_inv2, const double* __restrict__ nu_inv,
-                  Ctl* __restrict__ ctl, int p, unsigned long long seed) {
+scales_kernel(const double* __restrict__ beta, double* __restrict__ lam_inv2, double* __restrict__ nu_inv,
+              Ctl* __restrict__ ctl, int p, unsigned long long seed, int freeze_scales) {
   __shared__ double red[kScaleThreads];
   const int tid = threadIdx.x;
-  const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
-  const double tau_inv2 = ctl->tau_inv2;
+  const unsigned long long k = ctl->sweep + 1ull;
+  const uint32_t sweep = (uint32_t)k;
+  double* __restrict__ h_lambda = ctl->h_lambda;
+  double* __restrict__ h_tau = ctl->h_tau;
+  const unsigned long long hrow = k - 1ull - ctl->hist_base;
+  const double tau_old = ctl->tau_inv2;
   double s = 0.0;
   bool bad = false;
   for (int j = tid; j < p; j += kScaleThreads) {
-    const double u = uniform_a(seed, (unsigned long long)j, sweep, TAG_LAMBDA);
-    const double b = beta[j];
-    const double rate = nu_inv[j] + 0.5 * tau_inv2 * b * b;
-    const double l = -log(u) / rate;
-    lam_inv2[j] = l;
-    s += l * b * b;
-    bad |= !isfinite(l);
-  }
-  red[tid] = s;
-  __syncthreads();
-  for (int off = kScaleThreads / 2; off > 0; off >>= 1) {      // fixed tree: deterministic
-    if (tid < off) red[tid] += red[tid + off];
-    __syncthreads();
-  }
-  if (tid < 32) {
-    const double gam = cheng_gamma_warp(0.5 * ((double)p + 1.0), seed, sweep);
-    if (tid == 0) {
-      const double t = gam / (ctl->xi_inv + 0.5 * red[0]);
-      ctl->tau_inv2 = t;
-      if (!isfinite(t)) bad = true;
-    }
-  }
-  if (bad) atomicCAS(&ctl->status, 0, -5);
-}
-
-// e3 (nu^-1 and xi^-1 with beta, from the NEW lambda^-2, tau^-2), then g, then k <- k+1.
-__global__ void __launch_bounds__(kScaleThreads)
-scales_post_kernel(const double* __restrict__ beta, const double* __restrict__ lam_inv2, double* __restrict__ nu_inv,
-                   Ctl* __restrict__ ctl, int p, unsigned long long seed, int freeze_scales) {
-  const int tid = threadIdx.x;
-  double* __restrict__ h_beta = ctl->h_beta;
-  double* __restrict__ h_lambda = ctl->h_lambda;
-  double* __restrict__ h_tau = ctl->h_tau;
-  const unsigned long long k = ctl->sweep + 1ull;
-  const uint32_t sweep = (uint32_t)k;
-  const unsigned long long row = k - 1ull - ctl->hist_base;
-  const double tau_inv2 = ctl->tau_inv2;
-  bool bad = false;
-  for (int j = tid; j < p; j += kScaleThreads) {
-    const double l = lam_inv2[j];
+    double l = lam_inv2[j];
     if (!freeze_scales) {
-      const double u = uniform_a(seed, (unsigned long long)j, sweep, TAG_NU);
-      const double n = -log(u) / (1.0 + l);
+      const double u = uniform_a(seed, (unsigned long long)j, sweep, TAG_LAMBDA);
+      const double b = beta[j];
+      const double rate = nu_inv[j] + 0.5 * tau_old * b * b;
+      l = -log(u) / rate;
+      lam_inv2[j] = l;
+      s += l * b * b;
+      const double un = uniform_a(seed, (unsigned long long)j, sweep, TAG_NU);
+      const double n = -log(un) / (1.0 + l);
       nu_inv[j] = n;
-      bad |= !isfinite(n);
+      bad |= !isfinite(l) || !isfinite(n);
     }
-    if (h_beta != nullptr) {
-      h_beta[row * p + j] = beta[j];
-      h_lambda[row * p + j] = 1.0 / sqrt(l);
+    if (h_lambda != nullptr) h_lambda[hrow * (unsigned long long)p + j] = 1.0 / sqrt(l);
+  }
+  double tau_new = tau_old;
+  if (!freeze_scales) {
+    red[tid] = s;
+    __syncthreads();
+    for (int off = kScaleThreads / 2; off > 0; off >>= 1) {      // fixed tree: deterministic
+      if (tid < off) red[tid] += red[tid + off];
+      __syncthreads();
+    }
+    if (tid < 32) {
+      const double gam = cheng_gamma_warp(0.5 * ((double)p + 1.0), seed, sweep);
+      if (tid == 0) {
+        tau_new = gam / (ctl->xi_inv + 0.5 * red[0]);
+        ctl->tau_inv2 = tau_new;
+        const double u = uniform_a(seed, 0ull, sweep, TAG_XI);
+        const double x = -log(u) / (1.0 + tau_new);
+        ctl->xi_inv = x;
+        if (!isfinite(tau_new) || !isfinite(x)) bad = true;
+      }
     }
   }
-  if (tid == 0 && h_tau != nullptr) h_tau[row] = 1.0 / sqrt(tau_inv2);
+  if (tid == 0 && h_tau != nullptr) h_tau[hrow] = 1.0 / sqrt(tau_new);
   if (bad) atomicCAS(&ctl->status, 0, -5);
-  __syncthreads();
-  if (tid == 0) {
-    if (!freeze_scales) {
-      const double u = uniform_a(seed, 0ull, sweep, TAG_XI);
-      const double x = -log(u) / (1.0 + tau_inv2);
-      ctl->xi_inv = x;
-      if (!isfinite(x)) atomicCAS(&ctl->status, 0, -5);
-    }
-    ctl->sweep = k;
-  }
 }
 
 __global__ void validate_y_kernel(const unsigned char* __restrict__ y, long long N, int* __restrict__ bad) {
@@ -100,15 +80,9 @@ __global__ void side_kernel(const unsigned char* __restrict__ y, long long N, si
     side[i] = (signed char)(2 * (int)y[i] - 1);
 }
 
-cudaError_t scales_pre_launch(const double* beta, double* lam_inv2, const double* nu_inv, Ctl* ctl, int p,
-                              unsigned long long seed, cudaStream_t st) {
-  scales_pre_kernel<<<1, kScaleThreads, 0, st>>>(beta, lam_inv2, nu_inv, ctl, p, seed);
-  return cudaGetLastError();
-}
-
-cudaError_t scales_post_launch(const double* beta, const double* lam_inv2, double* nu_inv, Ctl* ctl, int p,
-                               unsigned long long seed, int freeze_scales, cudaStream_t st) {
-  scales_post_kernel<<<1, kScaleThreads, 0, st>>>(beta, lam_inv2, nu_inv, ctl, p, seed, freeze_scales);
+cudaError_t scales_launch(const double* beta, double* lam_inv2, double* nu_inv, Ctl* ctl, int p, unsigned long long seed,
+                          int freeze_scales, cudaStream_t st) {
+  scales_kernel<<<1, kScaleThreads, 0, st>>>(beta, lam_inv2, nu_inv, ctl, p, seed, freeze_scales);
   return cudaGetLastError();
 }
 

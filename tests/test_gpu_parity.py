@@ -71,8 +71,11 @@ def test_c5_shape_tma_f32_p2000_5_sweeps():
 
 @pytest.mark.parametrize("name,n_rows,p", [("C4", 3001, 4000), ("C4", 777, 3100), ("C5", 1501, 6000), ("C5", 901, 9000),
                                            ("C3", 4099, 640), ("C5", 300, 16000)])
-def test_fused_pass_only_wide_f32(name, n_rows, p):
-    """a1-a3 + b alone (scales and beta frozen at a planted state): z and X^T z against the oracle."""
+@pytest.mark.parametrize("eta_mode,z_tol", [(2, 2e-6), (1, 2e-6), (0, 1e-9)])
+def test_fused_pass_only_wide_f32(name, n_rows, p, eta_mode, z_tol, monkeypatch):
+    """a1-a3 + b alone (scales and beta frozen at a planted state): z and X^T z against the oracle, in the
+    three arithmetic modes of the eta phase (fp32 chains of 4 -> ~2e-7 in z; exact -> ~1e-13)."""
+    monkeypatch.setenv("HSP_FUSED_ETA", str(eta_mode))
     wl = hsp_synth.make(name, "cuda", n_rows=n_rows, p=p)
     Xh, yh = wl.host()
     beta = wl.beta_true * 0.7
@@ -86,9 +89,9 @@ def test_fused_pass_only_wide_f32(name, n_rows, p):
     zg, sg = g.get_latent(); zo, so = o.get_latent()
     assert np.array_equal(sg, so)
     ez, eg = mixed_err(zg, zo), mixed_err(g.get_xtz(), o.get_xtz())
-    print(name, n_rows, p, g.fused_variant(), "z", ez, "xtz", eg)
+    print(name, n_rows, p, g.fused_variant(), "eta mode", eta_mode, "z", ez, "xtz", eg)
     assert g.fused_variant() == "tma"
-    assert ez < 1e-9 and eg < 1e-5
+    assert ez < z_tol and eg < 1e-5
 
 
 @pytest.mark.parametrize("n_rows,p", [(4099, 256), (3001, 600), (1000, 1500), (513, 3000)])
