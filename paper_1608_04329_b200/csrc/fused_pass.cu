@@ -52,10 +52,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+// X is streamed once per sweep: its lines are marked evict-first in L2 so that the stream does not push out
+// the p x p working set of the concurrent Cholesky branch (L, W, Wt are re-read ~p/64 times per sweep).
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar, uint64_t pol) {
   asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
-      "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(dst_smem)),
+      "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
       : "memory");
 }
 
@@ -216,6 +224,7 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     if (lane == 0) {
       int st = 0;
       uint32_t ph = 0;
+      const uint64_t pol = l2_evict_first_policy();
       for (long long n = 0; n < my_tiles; ++n) {
         mbar_wait(&empty[st], ph ^ 1u);
         const long long row0 = (cta + n * grid) * RT;
@@ -223,7 +232,7 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         const uint32_t bytes = (uint32_t)((size_t)rows * row_bytes);
         mbar_arrive_expect_tx(&full[st], bytes);
         bulk_g2s(tiles + (size_t)st * stage_bytes, reinterpret_cast<const unsigned char*>(X) + (size_t)row0 * row_bytes,
-                 bytes, &full[st]);
+                 bytes, &full[st], pol);
         if (++st == S) { st = 0; ph ^= 1u; }
       }
     }
