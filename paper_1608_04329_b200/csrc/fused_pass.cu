@@ -59,6 +59,50 @@ __device__ __forceinline__ uint64_t l2_evict_first_policy() {
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
   return pol;
 }
+__device__ __forceinline__ void mbar_arrive_a(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_a(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred P1;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+      "@P1 bra DONE;\n\t"
+      "bra WAIT_LOOP;\n\t"
+      "DONE:\n\t"
+      "}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ float4 ld_shared_f32x4(uint32_t a) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float2 ld_shared_f32x2(uint32_t a) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float ld_shared_f32(uint32_t a) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ double2 ld_shared_f64x2(uint32_t a) {
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ double ld_shared_f64(uint32_t a) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void st_shared_f64(uint32_t a, double v) {
+  asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory");
+}
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar, uint64_t pol) {
   asm volatile(
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
@@ -75,7 +119,7 @@ template <> struct Vec<float> {
   static constexpr int V = 4;
   using Acc = float;
   float4 v;
-  __device__ __forceinline__ void load(const unsigned char* smem) { v = *reinterpret_cast<const float4*>(smem); }
+  __device__ __forceinline__ void load(uint32_t smem_addr) { v = ld_shared_f32x4(smem_addr); }
   __device__ __forceinline__ double dot(const double* b) const {
     double s = (double)v.x * b[0];
     s = fma((double)v.y, b[1], s);
@@ -102,7 +146,7 @@ template <> struct Vec<double> {
   static constexpr int V = 2;
   using Acc = double;
   double2 v;
-  __device__ __forceinline__ void load(const unsigned char* smem) { v = *reinterpret_cast<const double2*>(smem); }
+  __device__ __forceinline__ void load(uint32_t smem_addr) { v = ld_shared_f64x2(smem_addr); }
   __device__ __forceinline__ double dot(const double* b) const { return fma(v.y, b[1], v.x * b[0]); }
   __device__ __forceinline__ float dotf(const float*) const { return 0.f; }   // never used: fp64 X is always eta mode 0
   __device__ __forceinline__ void axpy(double z, double* acc) const {
@@ -142,50 +186,52 @@ static int env_int(const char* name, int dflt) {
   return (v && *v) ? atoi(v) : dflt;
 }
 
-constexpr int kComputeWarps = 8;                 // compute warps per row group (they cover one row's columns)
-constexpr int kComputeThreads = kComputeWarps * 32;
+constexpr int kComputeWarpsAll = 16;             // compute warps per CTA
+constexpr int kComputeThreadsAll = kComputeWarpsAll * 32;
 constexpr int kSamplerWarps = 4;
-__host__ __device__ constexpr int tma_threads(int G) { return (G * kComputeWarps + kSamplerWarps + 1) * 32; }
+constexpr int kTmaThreads = (kComputeWarpsAll + kSamplerWarps + 1) * 32;   // 672
 constexpr int kFlushRows = 16;   // fp32 x*z chains are flushed into the fp64 accumulators every >= 16 rows
 
 struct TmaSmemLayout {
   size_t tiles, eta_part, z64, z32, bars, total;
-  __host__ __device__ TmaSmemLayout(int S, int R, size_t stage_bytes) {
+  // WPR: warps that share one row (they cover its columns); R: rows per tile
+  __host__ __device__ TmaSmemLayout(int S, int R, int WPR, size_t stage_bytes) {
     tiles = 0;
     eta_part = tiles + (size_t)S * stage_bytes;
-    z64 = eta_part + (size_t)S * kComputeWarps * R * sizeof(double);
+    z64 = eta_part + (size_t)S * WPR * R * sizeof(double);
     z32 = z64 + (size_t)S * R * sizeof(double);
     bars = (z32 + (size_t)S * R * sizeof(float) + 15) & ~(size_t)15;
     total = bars + (size_t)4 * S * sizeof(uint64_t);
   }
 };
 
-// G row groups of 8 compute warps each: group g owns rows [g RT/G, (g+1) RT/G) of every tile (more
-// warps in flight per SM for the same tile shape; each group keeps its own X^T z accumulators and
-// writes its own partial row).
+// The 512 compute threads form 512/W row groups of W threads (W = 256 or 512).  Thread t of a group owns the
+// 16-byte column stripes (c*W + t)*V, c < C, of the rows [grp RT/G, (grp+1) RT/G) of every tile, keeps the
+// X^T z accumulators of those columns in registers for the whole kernel and writes its group's partial row.
+// Narrow rows (p <= 256 V) use two groups of 8 warps; wide rows one group of 16 warps, which halves the
+// per-thread column state (accumulators, beta) and keeps the kernel free of spills up to p = 8192 fp32.
 //
 // EM, the arithmetic of the eta phase for fp32 X (fp64 X is always mode 0):
 //   0  every element converted exactly to fp64, DFMA chain, fp64 butterfly       (z matches the oracle to ~1e-13)
-//   1  fp32 FMA chains of 4 elements, converted once per chain; fp64 butterfly   (~1e-7)
 //   2  fp32 FMA chains of 4 elements, fp32 butterfly, converted once per warp and row (~3e-7)
-// All three are far inside north_star's 1e-4 for fp32 X; 1 and 2 trade the 4 F2F.F64.F32 + 4 DFMA per
-// 16-byte vector (the conversion runs at a quarter of the FP64 rate through the MIO queue) for 4 FFMA.
-template <typename XT, int RT, int C, int G, int EM>
-__global__ void __launch_bounds__(tma_threads(G), 1)
+// Both are far inside north_star's 1e-4 for fp32 X; mode 2 trades the 4 F2F.F64.F32 + 4 DFMA per 16-byte vector
+// (the conversion runs at a quarter of the FP64 rate through the MIO queue and made the pass SM-bound) for 4 FFMA.
+template <typename XT, int RT, int C, int W, int EM>
+__global__ void __launch_bounds__(kTmaThreads, 1)
 fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
                unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
-               double* __restrict__ partial, double* __restrict__ z_out, int S, int D, long long n_tiles, int dbg) {
+               double* __restrict__ partial, double* __restrict__ z_out, int S, int D, long long n_tiles) {
   constexpr int V = Vec<XT>::V;
   using Acc = typename Vec<XT>::Acc;
   constexpr bool kF32 = sizeof(XT) == 4;
+  constexpr int G = kComputeThreadsAll / W;        // row groups
+  constexpr int WPR = W / 32;                      // warps per row
   constexpr int RG = RT / G;                       // rows of a tile per group
-  constexpr int kAllCompute = G * kComputeWarps;
-  constexpr int kThreads = tma_threads(G);
   static_assert(RT % G == 0 && RG >= 1, "rows per tile must split evenly over the groups");
   extern __shared__ __align__(128) unsigned char smem[];
   const size_t row_bytes = (size_t)p * sizeof(XT);
   const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
-  const TmaSmemLayout lay(S, RT, stage_bytes);
+  const TmaSmemLayout lay(S, RT, WPR, stage_bytes);
   unsigned char* tiles = smem + lay.tiles;
   double* eta_part = reinterpret_cast<double*>(smem + lay.eta_part);
   double* z64 = reinterpret_cast<double*>(smem + lay.z64);
@@ -203,8 +249,8 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
   if (tid == 0) {
     for (int s = 0; s < S; ++s) {
       mbar_init(&full[s], 1);
-      mbar_init(&empty[s], kAllCompute);
-      mbar_init(&eta_full[s], kAllCompute);
+      mbar_init(&empty[s], kComputeWarpsAll);
+      mbar_init(&eta_full[s], kComputeWarpsAll);
       mbar_init(&z_full[s], 1);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -213,13 +259,13 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
   // (stale or zero) and contribute x * 0 = 0 in the xz phase, so the inner loops need no row guards.
   {
     const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
-    for (size_t o = (size_t)tid * 16; o < (size_t)S * stage_bytes; o += (size_t)kThreads * 16)
+    for (size_t o = (size_t)tid * 16; o < (size_t)S * stage_bytes; o += (size_t)kTmaThreads * 16)
       *reinterpret_cast<uint4*>(tiles + o) = zero;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes before TMA writes
   }
   __syncthreads();
 
-  if (warp == kAllCompute + kSamplerWarps) {
+  if (warp == kComputeWarpsAll + kSamplerWarps) {
     // ===================== producer: one thread streams the tiles =====================
     if (lane == 0) {
       int st = 0;
@@ -236,11 +282,11 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         if (++st == S) { st = 0; ph ^= 1u; }
       }
     }
-  } else if (warp >= kAllCompute) {
+  } else if (warp >= kComputeWarpsAll) {
     // ===================== sampler warps: eta -> z, D tiles behind the eta phase =====================
     // Tile n goes to sampler warp n mod ns.  ns <= S keeps every mbarrier wait at most one phase
     // behind (a waiter two phases behind would alias on the parity bit).
-    const int sw = warp - kAllCompute;
+    const int sw = warp - kComputeWarpsAll;
     const int ns = S < kSamplerWarps ? S : kSamplerWarps;
     if (sw < ns) {
       // y is prefetched three tiles ahead: under a saturated HBM a lone 1-byte load takes microseconds
@@ -261,11 +307,11 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         mbar_wait(&eta_full[st], ph);
         double eta = 0.0;
         if (lane < RT) {
-          const double* ep = eta_part + (size_t)st * kComputeWarps * RT + lane;
+          const double* ep = eta_part + (size_t)st * WPR * RT + lane;
 #pragma unroll
-          for (int w = 0; w < kComputeWarps; ++w) eta += ep[w * RT];
+          for (int w = 0; w < WPR; ++w) eta += ep[w * RT];
         }
-        const double wpos = (dbg & 1) ? fabs(eta) + u : tnpos(ystar * eta, u);
+        const double wpos = tnpos(ystar * eta, u);
         const double z = valid ? ystar * wpos : 0.0;
         if (lane < RT) {
           z64[st * RT + lane] = z;
@@ -281,9 +327,9 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     }
   } else {
     // ===================== compute warps: eta partials, then x*z from the same stage =====================
-    // Thread t of a group owns the 16-byte column stripes (c*256 + t)*V.  Stripes past p read column 0
-    // with beta = 0 and are never written back, so the loops below are straight-line code.
-    const int grp = warp / kComputeWarps, wg = warp % kComputeWarps, gt = tid % kComputeThreads;
+    // Stripes past p read column 0 with beta = 0 and are never written back, so the loops below are
+    // straight-line code.  All shared-memory addresses are 32-bit and advance incrementally with the ring.
+    const int grp = tid / W, wg = (tid % W) >> 5, gt = tid % W;
     double breg[EM == 0 ? C : 1][V];
     float bregf[EM == 0 ? 1 : C][V];
     double acc64[C][V];
@@ -291,7 +337,7 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     uint32_t coff[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) {
-      const int col = (c * kComputeThreads + gt) * V;
+      const int col = (c * W + gt) * V;
       coff[c] = (col < p) ? (uint32_t)(col * sizeof(XT)) : 0u;
 #pragma unroll
       for (int v = 0; v < V; ++v) {
@@ -303,97 +349,95 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     }
     const int my_row = grp * RG + row_of_lane<RG>(lane);
     const bool writer = (lane & (32 / RG - 1)) == 0;
-    const uint32_t rb = (uint32_t)row_bytes;
-    const uint32_t goff = (uint32_t)(grp * RG) * rb;   // first row of this group inside a tile
+    const uint32_t rb = (uint32_t)row_bytes, sb = (uint32_t)stage_bytes;
+    const uint32_t tiles0 = smem_u32(tiles) + (uint32_t)(grp * RG) * rb;      // this group's first row, stage 0
+    const uint32_t tiles_end = tiles0 + (uint32_t)S * sb;
+    const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty), etaf0 = smem_u32(eta_full), zf0 = smem_u32(z_full);
+    const uint32_t epart0 = smem_u32(eta_part) + (uint32_t)((wg * RT + my_row) * sizeof(double));
+    const uint32_t zsrc0 = kF32 ? smem_u32(z32) + (uint32_t)(grp * RG * sizeof(float))
+                                : smem_u32(z64) + (uint32_t)(grp * RG * sizeof(double));
+    constexpr uint32_t kEpStride = WPR * RT * sizeof(double), kZStride = RT * (kF32 ? sizeof(float) : sizeof(double));
+    uint32_t tile_e = tiles0, tile_g = tiles0;
+    uint32_t st_e = 0, st_g = 0, ph_e = 0, ph_g = 0;
     int rows_since_flush = 0;
-    int st_e = 0, st_g = 0;
-    uint32_t ph_e = 0, ph_g = 0;
-    const int total_it = (int)my_tiles + D;
+    const int n_my = (int)my_tiles, total_it = n_my + D;
     for (int it = 0; it < total_it; ++it) {
-      if (it < (int)my_tiles) {
-        mbar_wait(&full[st_e], ph_e);
-        const unsigned char* tile = tiles + (size_t)st_e * stage_bytes + goff;
+      if (it < n_my) {
+        mbar_wait_a(full0 + 8u * st_e, ph_e);
         double tot;
         if constexpr (EM == 0) {
           double part[RG];
 #pragma unroll
           for (int r = 0; r < RG; ++r) part[r] = 0.0;
-          if (!(dbg & 2)) {
-#pragma unroll
-            for (int c = 0; c < C; ++c) {
-              Vec<XT> x[RG];
-#pragma unroll
-              for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
-#pragma unroll
-              for (int r = 0; r < RG; ++r) part[r] += x[r].dot(breg[c]);
-            }
-          }
-          tot = warp_reduce_rows<double, RG>(part, lane);
-        } else {
-          using PT = typename std::conditional<EM == 1, double, float>::type;
-          PT part[RG];
-#pragma unroll
-          for (int r = 0; r < RG; ++r) part[r] = (PT)0;
-          if (!(dbg & 2)) {
-#pragma unroll
-            for (int c = 0; c < C; ++c) {
-              Vec<XT> x[RG];
-#pragma unroll
-              for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
-#pragma unroll
-              for (int r = 0; r < RG; ++r) part[r] += (PT)x[r].dotf(bregf[c]);
-            }
-          }
-          tot = (double)warp_reduce_rows<PT, RG>(part, lane);
-        }
-        if (writer) eta_part[((size_t)st_e * kComputeWarps + wg) * RT + my_row] = tot;
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&eta_full[st_e]);
-        if (++st_e == S) { st_e = 0; ph_e ^= 1u; }
-      }
-      if (it >= D) {
-        mbar_wait(&z_full[st_g], ph_g);
-        const unsigned char* tile = tiles + (size_t)st_g * stage_bytes + goff;
-        Acc zr[RG];
-        if constexpr (kF32) {
-          const float* zp = z32 + st_g * RT + grp * RG;
-          if constexpr (RG % 4 == 0) {
-#pragma unroll
-            for (int q = 0; q < RG / 4; ++q) {
-              const float4 t = *reinterpret_cast<const float4*>(zp + 4 * q);
-              zr[4 * q] = t.x; zr[4 * q + 1] = t.y; zr[4 * q + 2] = t.z; zr[4 * q + 3] = t.w;
-            }
-          } else if constexpr (RG == 2) {
-            const float2 t = *reinterpret_cast<const float2*>(zp);
-            zr[0] = t.x; zr[1] = t.y;
-          } else {
-            zr[0] = zp[0];
-          }
-        } else {
-          const double* zp = z64 + st_g * RT + grp * RG;
-          if constexpr (RG % 2 == 0) {
-#pragma unroll
-            for (int q = 0; q < RG / 2; ++q) {
-              const double2 t = *reinterpret_cast<const double2*>(zp + 2 * q);
-              zr[2 * q] = t.x; zr[2 * q + 1] = t.y;
-            }
-          } else {
-            zr[0] = zp[0];
-          }
-        }
-        if (!(dbg & 4)) {
 #pragma unroll
           for (int c = 0; c < C; ++c) {
             Vec<XT> x[RG];
 #pragma unroll
-            for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
+            for (int r = 0; r < RG; ++r) x[r].load(tile_e + r * rb + coff[c]);
 #pragma unroll
-            for (int r = 0; r < RG; ++r) x[r].axpy(zr[r], acc[c]);
+            for (int r = 0; r < RG; ++r) part[r] += x[r].dot(breg[c]);
+          }
+          tot = warp_reduce_rows<double, RG>(part, lane);
+        } else {
+          float part[RG];
+#pragma unroll
+          for (int r = 0; r < RG; ++r) part[r] = 0.f;
+#pragma unroll
+          for (int c = 0; c < C; ++c) {
+            Vec<XT> x[RG];
+#pragma unroll
+            for (int r = 0; r < RG; ++r) x[r].load(tile_e + r * rb + coff[c]);
+#pragma unroll
+            for (int r = 0; r < RG; ++r) part[r] += x[r].dotf(bregf[c]);
+          }
+          tot = (double)warp_reduce_rows<float, RG>(part, lane);
+        }
+        if (writer) st_shared_f64(epart0 + st_e * kEpStride, tot);
+        __syncwarp();
+        if (lane == 0) mbar_arrive_a(etaf0 + 8u * st_e);
+        tile_e += sb;
+        if (++st_e == (uint32_t)S) { st_e = 0; ph_e ^= 1u; tile_e = tiles0; }
+      }
+      if (it >= D) {
+        mbar_wait_a(zf0 + 8u * st_g, ph_g);
+        Acc zr[RG];
+        const uint32_t zp = zsrc0 + st_g * kZStride;
+        if constexpr (kF32) {
+          if constexpr (RG % 4 == 0) {
+#pragma unroll
+            for (int q = 0; q < RG / 4; ++q) {
+              const float4 t = ld_shared_f32x4(zp + 16 * q);
+              zr[4 * q] = t.x; zr[4 * q + 1] = t.y; zr[4 * q + 2] = t.z; zr[4 * q + 3] = t.w;
+            }
+          } else if constexpr (RG == 2) {
+            const float2 t = ld_shared_f32x2(zp);
+            zr[0] = t.x; zr[1] = t.y;
+          } else {
+            zr[0] = ld_shared_f32(zp);
+          }
+        } else {
+          if constexpr (RG % 2 == 0) {
+#pragma unroll
+            for (int q = 0; q < RG / 2; ++q) {
+              const double2 t = ld_shared_f64x2(zp + 16 * q);
+              zr[2 * q] = t.x; zr[2 * q + 1] = t.y;
+            }
+          } else {
+            zr[0] = ld_shared_f64(zp);
           }
         }
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+          Vec<XT> x[RG];
+#pragma unroll
+          for (int r = 0; r < RG; ++r) x[r].load(tile_g + r * rb + coff[c]);
+#pragma unroll
+          for (int r = 0; r < RG; ++r) x[r].axpy(zr[r], acc[c]);
+        }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[st_g]);
-        if (++st_g == S) { st_g = 0; ph_g ^= 1u; }
+        if (lane == 0) mbar_arrive_a(empty0 + 8u * st_g);
+        tile_g += sb;
+        if (++st_g == (uint32_t)S) { st_g = 0; ph_g ^= 1u; tile_g = tiles0; }
         if constexpr (kF32) {
           rows_since_flush += RG;
           if (rows_since_flush >= kFlushRows) {
@@ -406,9 +450,10 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         }
       }
     }
+    (void)tiles_end;
 #pragma unroll
     for (int c = 0; c < C; ++c) {
-      const int col = (c * kComputeThreads + gt) * V;
+      const int col = (c * W + gt) * V;
 #pragma unroll
       for (int v = 0; v < V; ++v)
         if (col + v < p) partial[((size_t)cta * G + grp) * p + col + v] = acc64[c][v] + (double)acc[c][v];
@@ -521,51 +566,53 @@ reduce_partials_kernel(const double* __restrict__ partial, int n_part, int p, do
 // Host side: variant selection and launch
 // ------------------------------------------------------------------------------------------------
 
-static int round_chunks(int c) {
-  const int opts[] = {1, 2, 3, 4, 6, 8, 12, 16};
-  for (int o : opts) if (c <= o) return o;
-  return 0;
+// Tile shapes of the TMA kernel: W threads across a row, C 16-byte chunks per thread, RT rows per tile
+// (a stage is ~32 KB).  vec = 16-byte vectors per row.
+struct TmaShape { int RT, C, W; };
+static bool tma_shape(int vec, int prefer_w, TmaShape* out) {
+  const TmaShape shapes[] = {{8, 1, 256}, {4, 2, 256}, {4, 1, 512}, {2, 2, 512}, {1, 4, 512}, {1, 8, 512}};
+  for (const TmaShape& sh : shapes) {
+    if (vec > sh.C * sh.W) continue;
+    if (prefer_w && sh.W != prefer_w && vec <= 512 && vec > 256) continue;   // p in (256 V, 512 V]: two candidates
+    *out = sh;
+    return true;
+  }
+  return false;
 }
-static int rows_for_chunks(int c) { return c == 1 ? 8 : c == 2 ? 4 : c <= 4 ? 2 : 1; }
 
 FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X) {
   FusedPlan pl{};
   const size_t elem = dtype == kF32 ? 4 : 8;
-  const int V = (int)(16 / elem);
   const size_t row_bytes = (size_t)p * elem;
-  const int c_raw = (int)((p + V * kComputeThreads - 1) / (V * kComputeThreads));
-  const int C = round_chunks(c_raw);
   const bool aligned = (row_bytes % 16 == 0) && ((reinterpret_cast<uintptr_t>(X) & 15) == 0);
-  const bool wide = (p / V) >= kComputeThreads / 2;
+  const int vec = (int)(row_bytes / 16);
+  const bool wide = vec >= 128;
   const int force = env_int("HSP_FUSED_VARIANT", -1);
-  if (aligned && C != 0 && (wide || force == 1) && force != 0) {
-    const int RT = rows_for_chunks(C);
+  TmaShape sh{};
+  if (aligned && (wide || force == 1) && force != 0 && tma_shape(vec, env_int("HSP_FUSED_W", 0), &sh)) {
+    const int RT = sh.RT, WPR = sh.W / 32;
     const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
     const size_t budget = 227 * 1024;
     int S = env_int("HSP_FUSED_STAGES", 0);
     if (S <= 0) {
       S = 12;
-      while (S > 2 && TmaSmemLayout(S, RT, stage_bytes).total > budget) --S;
+      while (S > 2 && TmaSmemLayout(S, RT, WPR, stage_bytes).total > budget) --S;
     }
-    if (S >= 3 && TmaSmemLayout(S, RT, stage_bytes).total <= budget) {
+    if (S >= 3 && TmaSmemLayout(S, RT, WPR, stage_bytes).total <= budget) {
       int D = env_int("HSP_FUSED_LAG", 0);
       if (D <= 0) D = (S - 1) / 2;
       if (D > S - 2) D = S - 2;
       if (D < 1) D = 1;
       pl.variant = 1;
-      pl.rows_per_tile = RT; pl.chunks = C; pl.stages = S; pl.lag = D;
-      int G = env_int("HSP_FUSED_GROUPS", 2);
-      if (G != 1 && G != 2) G = 2;
-      if (RT % G != 0) G = 1;
-      pl.groups = G;
+      pl.rows_per_tile = RT; pl.chunks = sh.C; pl.width = sh.W; pl.stages = S; pl.lag = D;
+      pl.groups = kComputeThreadsAll / sh.W;
       int em = dtype == kF32 ? env_int("HSP_FUSED_ETA", 2) : 0;
-      if (em < 0 || em > 2 || G != ((RT % 2 == 0) ? 2 : 1)) em = 0;
-      pl.eta_mode = em;
+      pl.eta_mode = (em == 0) ? 0 : 2;
       pl.n_tiles = (N + RT - 1) / RT;
       int grid = env_int("HSP_FUSED_GRID", num_sms);
       if ((long long)grid > pl.n_tiles) grid = (int)pl.n_tiles;
-      pl.grid = grid; pl.block = tma_threads(G);
-      pl.smem = TmaSmemLayout(S, RT, stage_bytes).total;
+      pl.grid = grid; pl.block = kTmaThreads;
+      pl.smem = TmaSmemLayout(S, RT, WPR, stage_bytes).total;
       return pl;
     }
   }
@@ -578,11 +625,11 @@ FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X) 
   return pl;
 }
 
-template <typename XT, int RT, int C, int G, int EM>
+template <typename XT, int RT, int C, int W, int EM>
 static cudaError_t launch_tma(const FusedPlan& pl, const void* X, const unsigned char* y, long long N, int p,
                               unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                               double* z_out, cudaStream_t st) {
-  auto kern = fused_pass_tma<XT, RT, C, G, EM>;
+  auto kern = fused_pass_tma<XT, RT, C, W, EM>;
   static bool configured = false;   // per instantiation
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
@@ -591,7 +638,7 @@ static cudaError_t launch_tma(const FusedPlan& pl, const void* X, const unsigned
   }
   if (N < 0) return cudaSuccess;     // prepare-only call (sets the attribute outside stream capture)
   kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
-                                          pl.stages, pl.lag, pl.n_tiles, env_int("HSP_FUSED_DEBUG", 0));
+                                          pl.stages, pl.lag, pl.n_tiles);
   return cudaGetLastError();
 }
 
@@ -600,26 +647,19 @@ static cudaError_t dispatch_tma(const FusedPlan& pl, const void* X, const unsign
                                 unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                                 double* z_out, cudaStream_t st) {
 #define HSP_TMA_ARGS pl, X, y, N, p, seed, beta, ctl, partial, z_out, st
-#define HSP_TMA_CASE(RT_, C_)                                                                    \
-  case C_: {                                                                                     \
-    constexpr int G_ = ((RT_) % 2 == 0) ? 2 : 1;                                                 \
-    if constexpr (sizeof(XT) == 4) {                                                             \
-      if (pl.groups == G_ && pl.eta_mode == 1) return launch_tma<XT, RT_, C_, G_, 1>(HSP_TMA_ARGS); \
-      if (pl.groups == G_ && pl.eta_mode == 2) return launch_tma<XT, RT_, C_, G_, 2>(HSP_TMA_ARGS); \
-    }                                                                                            \
-    if (pl.groups == G_) return launch_tma<XT, RT_, C_, G_, 0>(HSP_TMA_ARGS);                    \
-    return launch_tma<XT, RT_, C_, 1, 0>(HSP_TMA_ARGS);                                          \
+#define HSP_TMA_CASE(RT_, C_, W_)                                                                  \
+  if (pl.rows_per_tile == RT_ && pl.chunks == C_ && pl.width == W_) {                              \
+    if constexpr (sizeof(XT) == 4) {                                                               \
+      if (pl.eta_mode == 2) return launch_tma<XT, RT_, C_, W_, 2>(HSP_TMA_ARGS);                   \
+    }                                                                                              \
+    return launch_tma<XT, RT_, C_, W_, 0>(HSP_TMA_ARGS);                                           \
   }
-  switch (pl.chunks) {
-    HSP_TMA_CASE(8, 1)
-    HSP_TMA_CASE(4, 2)
-    HSP_TMA_CASE(2, 3)
-    HSP_TMA_CASE(2, 4)
-    HSP_TMA_CASE(1, 6)
-    HSP_TMA_CASE(1, 8)
-    HSP_TMA_CASE(1, 12)
-    HSP_TMA_CASE(1, 16)
-  }
+  HSP_TMA_CASE(8, 1, 256)
+  HSP_TMA_CASE(4, 2, 256)
+  HSP_TMA_CASE(4, 1, 512)
+  HSP_TMA_CASE(2, 2, 512)
+  HSP_TMA_CASE(1, 4, 512)
+  HSP_TMA_CASE(1, 8, 512)
 #undef HSP_TMA_CASE
 #undef HSP_TMA_ARGS
   return cudaErrorInvalidValue;

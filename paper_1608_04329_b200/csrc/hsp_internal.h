@@ -28,7 +28,8 @@ struct FusedPlan {
   int rows_per_tile;  // R
   int stages;         // S
   int lag;            // D
-  int chunks;         // C
+  int chunks;         // C: 16-byte column chunks per compute thread
+  int width;          // W: compute threads across one row (256 or 512)
   int groups;         // G: row groups of compute warps (partial rows = grid * G)
   int eta_mode;       // EM: arithmetic of the eta phase for fp32 X (fused_pass.cu)
   long long n_tiles;

@@ -71,10 +71,10 @@ def test_c5_shape_tma_f32_p2000_5_sweeps():
 
 @pytest.mark.parametrize("name,n_rows,p", [("C4", 3001, 4000), ("C4", 777, 3100), ("C5", 1501, 6000), ("C5", 901, 9000),
                                            ("C3", 4099, 640), ("C5", 300, 16000)])
-@pytest.mark.parametrize("eta_mode,z_tol", [(2, 2e-6), (1, 2e-6), (0, 1e-9)])
+@pytest.mark.parametrize("eta_mode,z_tol", [(2, 2e-6), (0, 1e-9)])
 def test_fused_pass_only_wide_f32(name, n_rows, p, eta_mode, z_tol, monkeypatch):
     """a1-a3 + b alone (scales and beta frozen at a planted state): z and X^T z against the oracle, in the
-    three arithmetic modes of the eta phase (fp32 chains of 4 -> ~2e-7 in z; exact -> ~1e-13)."""
+    two arithmetic modes of the eta phase (fp32 chains of 4 -> ~2e-7 in z; exact -> ~1e-13)."""
     monkeypatch.setenv("HSP_FUSED_ETA", str(eta_mode))
     wl = hsp_synth.make(name, "cuda", n_rows=n_rows, p=p)
     Xh, yh = wl.host()
