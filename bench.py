@@ -154,6 +154,7 @@ def main():
     import torch.distributed as dist
     import hsp_synth
     import paper_1608_04329_b200 as hsp
+    from paper_1608_04329_b200 import multi
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
@@ -164,7 +165,7 @@ def main():
 
     # Multi-GPU: independent chains, one per GPU, same data recipe, seed + rank.
     wl = hsp_synth.make(args.workload, dev)
-    seed = wl.seed + rank
+    seed = multi.chain_seed(wl.seed, rank)
     stream = torch.cuda.Stream(device=dev)
     x_bytes = wl.X.numel() * wl.X.element_size()
     with torch.cuda.stream(stream):
@@ -194,11 +195,8 @@ def main():
         # sanity: the chain is finite and moving
         b, lam, tau = chain.get_draws()
         assert np.all(np.isfinite(b)) and np.all(np.isfinite(lam)) and np.all(tau > 0)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * args.steps / (ms * 1e-3)
+    ms = multi.max_over_ranks(ms, dev)
+    value = multi.whole_job_rate(args.steps, ms)
 
     line = None
     if rank == 0:
@@ -253,10 +251,7 @@ def main():
         torch.cuda.synchronize(dev)
         dt = time.perf_counter() - t0
         c2.close()
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = multi.max_over_ranks(dt, dev)
         if rank == 0:
             line["e2e"] = {"value": world * e2e_steps / dt, "unit": "sweeps/s",
                            "h2d_bytes_per_step": (x_bytes + wl.N) / e2e_steps, "d2h_bytes_per_step": (2 * wl.p + 1) * 8,

@@ -1,0 +1,55 @@
+"""Multi-GPU plumbing: one process per GPU, one independent chain per rank
+(seed + rank), no data-path collective.  torch.distributed is used only for the timing reduction and for
+gathering the draws of all chains (convergence diagnostics across chains).  Nothing here touches the
+sampler's arithmetic; it works on any backend (nccl on GPUs, gloo in the CPU tests)."""
+import torch
+import torch.distributed as dist
+
+
+def world():
+    """(rank, world_size) of the default process group, (0, 1) when none is initialised."""
+    if dist.is_available() and dist.is_initialized():
+        return dist.get_rank(), dist.get_world_size()
+    return 0, 1
+
+
+def chain_seed(base_seed, rank):
+    """Philox seed of the chain on `rank`: distinct keys give independent streams (counter-based RNG)."""
+    return (int(base_seed) + int(rank)) & 0xFFFFFFFFFFFFFFFF
+
+
+def max_over_ranks(value, device="cpu"):
+    """Device-timed milliseconds -> the maximum over ranks (the job is as slow as its slowest rank)."""
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    if world()[1] > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank, ms_max):
+    """Whole-job throughput: units all ranks processed / the slowest rank's time."""
+    return world()[1] * units_per_rank / (ms_max * 1e-3)
+
+
+def gather_draws(draws):
+    """draws: tensor [n_iter, d] of this rank's chain -> tensor [world, n_iter, d] on every rank."""
+    draws = draws.contiguous()
+    _, ws = world()
+    if ws == 1:
+        return draws.unsqueeze(0)
+    out = [torch.empty_like(draws) for _ in range(ws)]
+    dist.all_gather(out, draws)
+    return torch.stack(out)
+
+
+def split_rhat(chains):
+    """Split-R-hat of Gelman et al. per coordinate; chains: [m, n, d] (m chains of n draws).  Each chain is
+    split in two halves, so the statistic also detects a drifting single chain."""
+    m, n, d = chains.shape
+    h = n // 2
+    x = torch.cat([chains[:, :h], chains[:, h:2 * h]], dim=0).to(torch.float64)     # [2m, h, d]
+    means = x.mean(dim=1)
+    W = x.var(dim=1, unbiased=True).mean(dim=0)
+    B = h * means.var(dim=0, unbiased=True)
+    var_plus = (h - 1) / h * W + B / h
+    return torch.sqrt(var_plus / W)
