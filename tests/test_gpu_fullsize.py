@@ -98,7 +98,11 @@ def test_full_size_sweep_against_oracle(name, warm):
     G_ref = gram_fp64(wl.X)
     e_gram = float(np.max(np.abs(np.tril(Gg) - np.tril(G_ref))) / np.max(np.abs(G_ref)))
     Q = G_ref + np.diag(so["tau_inv2"] * so["lam_inv2"])
-    L = np.linalg.cholesky(Q) if p > 2000 else oracle.cholesky_lower(Q)
+    if p > 2000:
+        L = np.linalg.cholesky(Q)
+    else:
+        rc, L = oracle.cholesky_lower(Q)
+        assert rc == 0
     e = np.asarray(oracle.norm_inv_many(np.asarray(oracle.uniforms_many(seed, np.arange(p, dtype=np.uint64), k, 3)[0])))
     if p > 2000:
         import scipy.linalg as sl
