@@ -138,6 +138,7 @@ def main():
     ap.add_argument("--workload", default="C3", choices=list(WORKLOAD_DESC))
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--paper-design", action="store_true", help="A/B: rows a1-a3 by the paper's own decomposition (two X reads, rejection sampler)")
     ap.add_argument("--graph", action="store_true", help="replay the captured CUDA graph in the timed region (no per-kernel events)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -170,7 +171,7 @@ def main():
     x_bytes = wl.X.numel() * wl.X.element_size()
     with torch.cuda.stream(stream):
         chain = hsp.HorseshoeProbit(wl.X, wl.y, seed, stream=stream)
-        chain.set_flags(0 if args.graph else hsp.HSP_NO_GRAPH)
+        chain.set_flags((0 if args.graph else hsp.HSP_NO_GRAPH) | (hsp.HSP_PAPER_DESIGN if args.paper_design else 0))
         chain.sweep(args.warmup)
         chain.sync()
         chain.fused_pass_ms()                     # reset the event accumulator
@@ -210,7 +211,7 @@ def main():
             if os.path.exists(tp):
                 with open(tp) as f:
                     traffic = json.load(f).get(args.workload)
-            roofline = {"bound": "hbm", "kernel": f"fused_pass_{variant}", "achieved": achieved, "peak": peaks["hbm_gbs"],
+            roofline = {"bound": "hbm", "kernel": "paper_design(gemv+rejection+gemvT)" if args.paper_design else f"fused_pass_{variant}", "achieved": achieved, "peak": peaks["hbm_gbs"],
                         "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)", "unit": "GB/s",
                         "frac": achieved / peaks["hbm_gbs"], "frac_of_8TBps": achieved / 8000.0, "traffic": traffic,
                         "alg_bytes_per_launch": alg_bytes, "avg_launch_ms": fused_ms, "launches_timed": fused_n,

@@ -49,7 +49,10 @@ enum {
   HSP_FREEZE_Z = 4u,      /* skip a1-a3 and b (g keeps the value of the last sweep that ran them)   */
   HSP_FREEZE_BETA = 16u,  /* skip c, d1, d2 (beta keeps its current value)                          */
   HSP_NO_GRAPH = 32u,     /* enqueue kernels directly instead of replaying the captured CUDA graph  */
-  HSP_SERIAL = 64u        /* one stream: no overlap of the Cholesky branch with the fused pass      */
+  HSP_SERIAL = 64u,       /* one stream: no overlap of the Cholesky branch with the fused pass      */
+  HSP_PAPER_DESIGN = 128u /* A/B: rows a1-a3 by the paper's own decomposition: X beta, a
+                             divergent rejection sampler (thread per row), X^T z -- X is read twice, mu and z go
+                             through HBM; same law as the fused pass, different draws (implies HSP_STORE_Z)       */
 };
 
 /* Create a chain.  PAPER.md:186 (X, y), PAPER.md:289 (cold start), PAPER.md:195 (X^T X once).

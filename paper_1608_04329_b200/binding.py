@@ -11,6 +11,7 @@ from . import build as _build
 HSP_F32, HSP_F64 = 0, 1
 HSP_OK, HSP_EINVAL, HSP_ENOMEM, HSP_ECUDA, HSP_ENOTPD, HSP_ENUMERIC = 0, -1, -2, -3, -4, -5
 HSP_STORE_Z, HSP_FREEZE_SCALES, HSP_FREEZE_Z, HSP_FREEZE_BETA, HSP_NO_GRAPH, HSP_SERIAL = 1, 2, 4, 16, 32, 64
+HSP_PAPER_DESIGN = 128
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _HEADER = os.path.join(os.path.dirname(_HERE), "include", "hsp.h")

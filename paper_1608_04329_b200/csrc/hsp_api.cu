@@ -10,6 +10,7 @@
 #include <cstring>
 #include <string>
 #include <vector>
+#include <algorithm>
 #include <new>
 #include "../../include/hsp.h"
 #include "hsp_device.cuh"
@@ -36,7 +37,8 @@ struct hsp_state {
   unsigned flags = 0; int num_sms = 0;
   void* own_X = nullptr; unsigned char* own_y = nullptr;
   double *G = nullptr, *L = nullptr, *W = nullptr, *Wt = nullptr, *beta = nullptr, *lam_inv2 = nullptr,
-         *nu_inv = nullptr, *g = nullptr, *tv = nullptr, *partial = nullptr, *z = nullptr;
+         *nu_inv = nullptr, *g = nullptr, *tv = nullptr, *partial = nullptr, *z = nullptr, *mu = nullptr;
+  int pd_ctas = 0;                   // CTAs (= partial rows) of the paper-design X^T z product
   CholPlan chol{};
   signed char* side = nullptr;
   Ctl* ctl = nullptr;
@@ -60,7 +62,7 @@ static void free_state(hsp_state* s) {
   if (s->stream2) cudaStreamDestroy(s->stream2);
   if (s->own_stream) cudaStreamDestroy(s->own_stream);
   void* ptrs[] = {s->own_X, s->own_y, s->G, s->L, s->W, s->Wt, s->beta, s->lam_inv2, s->nu_inv, s->g, s->tv, s->partial,
-                  s->z, s->side, s->ctl, s->h_beta, s->h_lambda, s->h_tau};
+                  s->z, s->mu, s->side, s->ctl, s->h_beta, s->h_lambda, s->h_tau};
   for (void* q : ptrs) if (q) cudaFree(q);
   chol_plan_destroy(&s->chol);
   delete s;
@@ -103,8 +105,14 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
       }
       CK(cudaEventRecord(s->tev[s->tev_used], A));
     }
-    CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, s->N, s->p, s->seed, s->beta, s->ctl, s->partial,
-                         (s->flags & HSP_STORE_Z) ? s->z : nullptr, A));
+    if (s->flags & HSP_PAPER_DESIGN) {
+      CK(paper_design_launch(s->X, s->dtype, s->y, s->N, s->p, s->seed, s->beta, s->ctl, s->mu, s->z, s->partial,
+                             s->pd_ctas, s->num_sms, A));
+      *kernels += 2;
+    } else {
+      CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, s->N, s->p, s->seed, s->beta, s->ctl, s->partial,
+                           (s->flags & HSP_STORE_Z) ? s->z : nullptr, A));
+    }
     if (timed) { CK(cudaEventRecord(s->tev[s->tev_used + 1], A)); s->tev_used += 2; }
     *kernels += 1;
   }
@@ -113,7 +121,11 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
     CK(cudaEventRecord(s->ev_join, B));
     CK(cudaStreamWaitEvent(A, s->ev_join, 0));      // before the reduce: the tail kernels then chain by PDL
   }
-  if (do_z) { CK(reduce_partials_launch(s->partial, s->plan.grid * s->plan.groups, s->p, s->g, A)); *kernels += 1; }
+  if (do_z) {
+    const int n_part = (s->flags & HSP_PAPER_DESIGN) ? s->pd_ctas : s->plan.grid * s->plan.groups;
+    CK(reduce_partials_launch(s->partial, n_part, s->p, s->g, A));
+    *kernels += 1;
+  }
   if (do_beta) CK(beta_solve_launch(s->W, s->Wt, s->g, s->tv, s->beta, s->p, s->seed, s->ctl, A, kernels));
   else { CK(beta_keep_launch(s->beta, s->p, s->ctl, A)); *kernels += 1; }
   return HSP_OK;
@@ -163,7 +175,8 @@ static int create_common(hsp_state** out, hsp_state* s) {
   CK(cudaMalloc(&s->G, pp)); CK(cudaMalloc(&s->L, PP)); CK(cudaMalloc(&s->W, PP)); CK(cudaMalloc(&s->Wt, PP));
   CK(cudaMalloc(&s->beta, pv)); CK(cudaMalloc(&s->lam_inv2, pv)); CK(cudaMalloc(&s->nu_inv, pv));
   CK(cudaMalloc(&s->g, Pv)); CK(cudaMalloc(&s->tv, Pv));     // padded to P with zeros (the GEMVs read whole tiles)
-  CK(cudaMalloc(&s->partial, (size_t)s->plan.grid * s->plan.groups * pv));
+  s->pd_ctas = paper_design_ctas(N, s->num_sms);
+  CK(cudaMalloc(&s->partial, (size_t)std::max(s->plan.grid * s->plan.groups, s->pd_ctas) * pv));
   CK(cudaMalloc(&s->ctl, sizeof(Ctl)));
   // validate y in {0,1}
   int* bad = nullptr;
@@ -264,8 +277,11 @@ int hsp_destroy(hsp_state* s) {
 
 int hsp_set_flags(hsp_state* s, unsigned flags) {
   if (!s) return fail(HSP_EINVAL, "state is NULL");
-  const unsigned known = HSP_STORE_Z | HSP_FREEZE_SCALES | HSP_FREEZE_Z | HSP_FREEZE_BETA | HSP_NO_GRAPH | HSP_SERIAL;
+  const unsigned known = HSP_STORE_Z | HSP_FREEZE_SCALES | HSP_FREEZE_Z | HSP_FREEZE_BETA | HSP_NO_GRAPH | HSP_SERIAL |
+                         HSP_PAPER_DESIGN;
   if (flags & ~known) return fail(HSP_EINVAL, "unknown flag");
+  if (flags & HSP_PAPER_DESIGN) flags |= HSP_STORE_Z;   // the paper's design materialises z (and mu) in HBM
+  if ((flags & HSP_PAPER_DESIGN) && !s->mu) CK(cudaMalloc(&s->mu, (size_t)s->N * sizeof(double)));
   if ((flags & HSP_STORE_Z) && !s->z) {
     CK(cudaMalloc(&s->z, (size_t)s->N * sizeof(double)));
     CK(cudaMemsetAsync(s->z, 0, (size_t)s->N * sizeof(double), s->stream));

@@ -42,6 +42,12 @@ cudaError_t fused_pass_launch(const FusedPlan& plan, const void* X, int dtype, c
                               double* z_out, cudaStream_t st);
 cudaError_t reduce_partials_launch(const double* partial, int n_part, int p, double* g, cudaStream_t st);
 
+// ---- the paper's own decomposition of a1-a3 (two products + rejection sampler), for the A/B: paper_design.cu
+int paper_design_ctas(long long N, int num_sms);
+cudaError_t paper_design_launch(const void* X, int dtype, const unsigned char* y, long long N, int p, unsigned long long seed,
+                                const double* beta, const Ctl* ctl, double* mu, double* z, double* partial, int n_part,
+                                int num_sms, cudaStream_t st);
+
 // ---- Gram (c0): gram.cu
 cudaError_t gram_launch(const void* X, int dtype, long long N, int p, double* G, double* scratch, int splits,
                         cudaStream_t st);
