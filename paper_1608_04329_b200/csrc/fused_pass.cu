@@ -462,6 +462,226 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
 }
 
 // ------------------------------------------------------------------------------------------------
+// Narrow rows (fewer than 128 16-byte vectors per row, any p: the rows need not be a multiple of 16 bytes --
+// config C2, and the shape of the paper's real-data run, N = 1.3e6, p = 141).
+// Same pipeline as fused_pass_tma (producer / 16 compute warps / sampler warps, S-stage ring, lag D), but a tile
+// holds RT = 32..256 whole rows (RT a multiple of 32, so a tile starts 16-byte aligned and is a whole number of
+// 16-byte units) and the thread mappings differ:
+//   eta phase   L = 2^k lanes share a row (E = ceil(p / L) <= EMAX elements per lane, beta in registers); the
+//               512 compute threads cover 512/L rows per pass; shuffle reduction over the L lanes.
+//   xz phase    thread t owns column t mod p for the rows r = t div p (mod NG), NG = floor(512 / p) row groups;
+//               the NG accumulators of a column are combined through shared memory at the end (fixed order).
+//   sampler     a sampler warp takes a whole tile: lane = row, RT/32 batches.
+// The ragged last tile may not be a multiple of 16 bytes: the producer copies the 16-byte units by TMA and the
+// last < 16 bytes with plain loads.
+// ------------------------------------------------------------------------------------------------
+constexpr int kNarrowSamplers = 8;
+constexpr int kNarrowThreads = (kComputeWarpsAll + kNarrowSamplers + 1) * 32;   // 800
+
+struct NarrowSmemLayout {
+  size_t tiles, eta, z64, z32, red, bars, total;
+  __host__ __device__ NarrowSmemLayout(int S, int RT, int p, size_t stage_bytes) {
+    tiles = 0;
+    eta = tiles + (size_t)S * stage_bytes;
+    z64 = eta + (size_t)S * RT * sizeof(double);
+    z32 = z64 + (size_t)S * RT * sizeof(double);
+    red = (z32 + (size_t)S * RT * sizeof(float) + 15) & ~(size_t)15;
+    bars = red + (size_t)kComputeThreadsAll * sizeof(double);
+    total = bars + (size_t)4 * S * sizeof(uint64_t);
+    (void)p;
+  }
+};
+
+template <typename XT> __device__ __forceinline__ XT ld_shared_x(uint32_t a);
+template <> __device__ __forceinline__ float ld_shared_x<float>(uint32_t a) { return ld_shared_f32(a); }
+template <> __device__ __forceinline__ double ld_shared_x<double>(uint32_t a) { return ld_shared_f64(a); }
+
+template <typename XT, int EMAX, int EM>
+__global__ void __launch_bounds__(kNarrowThreads, 1)
+fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
+                  unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
+                  double* __restrict__ partial, double* __restrict__ z_out, int S, int D, int RT, int L,
+                  long long n_tiles) {
+  constexpr bool kF32 = sizeof(XT) == 4;
+  using Acc = typename std::conditional<kF32, float, double>::type;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const size_t row_bytes = (size_t)p * sizeof(XT);
+  const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
+  const NarrowSmemLayout lay(S, RT, p, stage_bytes);
+  unsigned char* tiles = smem + lay.tiles;
+  double* eta_s = reinterpret_cast<double*>(smem + lay.eta);
+  double* z64 = reinterpret_cast<double*>(smem + lay.z64);
+  float* z32 = reinterpret_cast<float*>(smem + lay.z32);
+  double* red = reinterpret_cast<double*>(smem + lay.red);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + lay.bars);
+  uint64_t* empty = full + S;
+  uint64_t* eta_full = empty + S;
+  uint64_t* z_full = eta_full + S;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const long long cta = blockIdx.x, grid = gridDim.x;
+  const long long my_tiles = cta < n_tiles ? (n_tiles - cta + grid - 1) / grid : 0;
+  const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
+
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], kComputeWarpsAll);
+      mbar_init(&eta_full[s], kComputeWarpsAll);
+      mbar_init(&z_full[s], 1);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  {
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+    for (size_t o = (size_t)tid * 16; o < (size_t)S * stage_bytes; o += (size_t)kNarrowThreads * 16)
+      *reinterpret_cast<uint4*>(tiles + o) = zero;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp == kComputeWarpsAll + kNarrowSamplers) {
+    // ===================== producer =====================
+    if (lane == 0) {
+      int st = 0;
+      uint32_t ph = 0;
+      const uint64_t pol = l2_evict_first_policy();
+      for (long long n = 0; n < my_tiles; ++n) {
+        mbar_wait(&empty[st], ph ^ 1u);
+        const long long row0 = (cta + n * grid) * RT;
+        const long long rows = (N - row0) < RT ? (N - row0) : RT;
+        const size_t bytes = (size_t)rows * row_bytes;
+        const uint32_t bulk = (uint32_t)(bytes & ~(size_t)15);
+        const unsigned char* src = reinterpret_cast<const unsigned char*>(X) + (size_t)row0 * row_bytes;
+        unsigned char* dst = tiles + (size_t)st * stage_bytes;
+        for (size_t b = bulk; b < bytes; ++b) dst[b] = src[b];       // ragged last tile only: < 16 bytes
+        if (bulk) {
+          mbar_arrive_expect_tx(&full[st], bulk);
+          bulk_g2s(dst, src, bulk, &full[st], pol);
+        } else {
+          mbar_arrive(&full[st]);
+        }
+        if (++st == S) { st = 0; ph ^= 1u; }
+      }
+    }
+  } else if (warp >= kComputeWarpsAll) {
+    // ===================== sampler warps: a whole tile each, lane = row =====================
+    const int sw = warp - kComputeWarpsAll;
+    const int ns = S < kNarrowSamplers ? S : kNarrowSamplers;
+    if (sw < ns) {
+      int st = sw;
+      uint32_t ph = 0;
+      for (long long n = sw; n < my_tiles; n += ns) {
+        const long long row0 = (cta + n * grid) * RT;
+        bool waited = false;
+        for (int b = 0; b < RT; b += 32) {
+          const long long i = row0 + b + lane;
+          const bool valid = i < N;
+          const int yi = valid ? (int)y[i] : 1;
+          const double u = uniform_a(seed, (unsigned long long)(valid ? i : 0), sweep, TAG_Z);
+          const double ystar = 2.0 * (double)yi - 1.0;
+          if (!waited) { mbar_wait(&eta_full[st], ph); waited = true; }
+          const double eta = eta_s[st * RT + b + lane];
+          const double wpos = tnpos(ystar * eta, u);
+          const double z = valid ? ystar * wpos : 0.0;
+          z64[st * RT + b + lane] = z;
+          z32[st * RT + b + lane] = (float)z;
+          if (valid && z_out != nullptr) z_out[i] = z;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&z_full[st]);
+        st += ns;
+        if (st >= S) { st -= S; ph ^= 1u; }
+      }
+    }
+  } else {
+    // ===================== compute warps =====================
+    // eta mapping: lane group of L lanes per row
+    const int l = tid & (L - 1), rsub = tid / L, rows_per_pass = kComputeThreadsAll / L;
+    double bd[kF32 && EM != 0 ? 1 : EMAX];
+    float bf[kF32 && EM != 0 ? EMAX : 1];
+#pragma unroll
+    for (int e = 0; e < EMAX; ++e) {
+      const int j = l + e * L;
+      const double bv = (j < p) ? beta[j] : 0.0;
+      if constexpr (kF32 && EM != 0) bf[e] = (float)bv; else bd[e] = bv;
+    }
+    // xz mapping: thread t -> column t mod p, row group t div p
+    const int NG = kComputeThreadsAll / p > 0 ? kComputeThreadsAll / p : 1;   // p <= 512 here
+    const int xg = tid / p, xj = tid - xg * p;
+    const bool xz_on = xg < NG;
+    double acc64 = 0.0;
+    Acc acc = (Acc)0;
+    const uint32_t rb = (uint32_t)row_bytes, sb = (uint32_t)stage_bytes;
+    const uint32_t tiles0 = smem_u32(tiles);
+    const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty), etaf0 = smem_u32(eta_full), zf0 = smem_u32(z_full);
+    uint32_t st_e = 0, st_g = 0, ph_e = 0, ph_g = 0;
+    int rows_since_flush = 0;
+    const int n_my = (int)my_tiles, total_it = n_my + D;
+    for (int it = 0; it < total_it; ++it) {
+      if (it < n_my) {
+        mbar_wait_a(full0 + 8u * st_e, ph_e);
+        const uint32_t tile = tiles0 + st_e * sb;
+        for (int r = rsub; r < RT; r += rows_per_pass) {
+          const uint32_t xa = tile + (uint32_t)r * rb + (uint32_t)l * (uint32_t)sizeof(XT);
+          double s;
+          if constexpr (kF32 && EM != 0) {
+            float c = 0.f;
+#pragma unroll
+            for (int e = 0; e < EMAX; ++e)
+              if (l + e * L < p) c = fmaf(ld_shared_f32(xa + (uint32_t)(e * L) * 4u), bf[e], c);
+#pragma unroll 1
+            for (int off = L >> 1; off >= 1; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
+            s = (double)c;
+          } else {
+            s = 0.0;
+#pragma unroll
+            for (int e = 0; e < EMAX; ++e)
+              if (l + e * L < p) s = fma((double)ld_shared_x<XT>(xa + (uint32_t)(e * L) * (uint32_t)sizeof(XT)), bd[e], s);
+#pragma unroll 1
+            for (int off = L >> 1; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+          }
+          if (l == 0) eta_s[st_e * RT + r] = s;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive_a(etaf0 + 8u * st_e);
+        if (++st_e == (uint32_t)S) { st_e = 0; ph_e ^= 1u; }
+      }
+      if (it >= D) {
+        mbar_wait_a(zf0 + 8u * st_g, ph_g);
+        if (xz_on) {
+          const uint32_t xa = tiles0 + st_g * sb + (uint32_t)xj * (uint32_t)sizeof(XT);
+          if constexpr (kF32) {
+            const float* zp = z32 + st_g * RT;
+#pragma unroll 4
+            for (int r = xg; r < RT; r += NG) acc = fmaf(ld_shared_f32(xa + (uint32_t)r * rb), zp[r], acc);
+          } else {
+            const double* zp = z64 + st_g * RT;
+#pragma unroll 4
+            for (int r = xg; r < RT; r += NG) acc = fma(ld_shared_f64(xa + (uint32_t)r * rb), zp[r], acc);
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive_a(empty0 + 8u * st_g);
+        if (++st_g == (uint32_t)S) { st_g = 0; ph_g ^= 1u; }
+        if constexpr (kF32) {
+          rows_since_flush += (RT + NG - 1) / NG;
+          if (rows_since_flush >= kFlushRows) { rows_since_flush = 0; acc64 += (double)acc; acc = 0.f; }
+        }
+      }
+    }
+    // combine the NG row groups of every column in fixed order (named barrier over the 16 compute warps)
+    red[tid] = acc64 + (double)acc;
+    asm volatile("bar.sync 1, %0;" ::"n"(kComputeThreadsAll) : "memory");
+    if (tid < p) {
+      double s = 0.0;
+      for (int g = 0; g < NG; ++g) s += red[g * p + tid];
+      partial[(size_t)cta * p + tid] = s;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Generic kernel: any p / alignment.  256-row tiles; phase 1 thread-per-row, phase 2 thread-per-column.
 // ------------------------------------------------------------------------------------------------
 constexpr int kGenThreads = 256;
@@ -580,6 +800,80 @@ static bool tma_shape(int vec, int prefer_w, TmaShape* out) {
   return false;
 }
 
+static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* X, FusedPlan* pl) {
+  const size_t elem = dtype == kF32 ? 4 : 8;
+  const size_t row_bytes = (size_t)p * elem;
+  // tiny problems (C1) are launch-bound: the generic kernel has no 224 KB ring to set up
+  if ((reinterpret_cast<uintptr_t>(X) & 15) != 0 || p > kComputeThreadsAll - 1 || (size_t)N * row_bytes < ((size_t)2 << 20)) return false;
+  int L = 1;
+  while (L < 32 && (p + L - 1) / L > 4) L <<= 1;
+  const int E = (p + L - 1) / L;
+  if (E > 16) return false;
+  int RT = (int)(32768 / row_bytes) / 32 * 32;
+  RT = RT < 32 ? 32 : RT > 256 ? 256 : RT;
+  if (env_int("HSP_NARROW_RT", 0) > 0) RT = env_int("HSP_NARROW_RT", 0) / 32 * 32;
+  const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
+  const size_t budget = 227 * 1024;
+  int S = env_int("HSP_FUSED_STAGES", 0);
+  if (S <= 0) {
+    S = 8;
+    while (S > 2 && NarrowSmemLayout(S, RT, p, stage_bytes).total > budget) --S;
+  }
+  if (S < 3 || NarrowSmemLayout(S, RT, p, stage_bytes).total > budget) return false;
+  int D = env_int("HSP_FUSED_LAG", 0);
+  if (D <= 0) D = (S - 1) / 2;
+  if (D > S - 2) D = S - 2;
+  if (D < 1) D = 1;
+  pl->variant = 2;
+  pl->rows_per_tile = RT; pl->chunks = E <= 4 ? 4 : E <= 8 ? 8 : 16; pl->width = L; pl->stages = S; pl->lag = D;
+  pl->groups = 1;
+  int em = dtype == kF32 ? env_int("HSP_FUSED_ETA", 2) : 0;
+  pl->eta_mode = (em == 0) ? 0 : 2;
+  pl->n_tiles = (N + RT - 1) / RT;
+  int grid = env_int("HSP_FUSED_GRID", num_sms);
+  if ((long long)grid > pl->n_tiles) grid = (int)pl->n_tiles;
+  pl->grid = grid; pl->block = kNarrowThreads;
+  pl->smem = NarrowSmemLayout(S, RT, p, stage_bytes).total;
+  return true;
+}
+
+template <typename XT, int EMAX, int EM>
+static cudaError_t launch_narrow(const FusedPlan& pl, const void* X, const unsigned char* y, long long N, int p,
+                                 unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
+                                 double* z_out, cudaStream_t st) {
+  auto kern = fused_pass_narrow<XT, EMAX, EM>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  if (N < 0) return cudaSuccess;
+  kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
+                                          pl.stages, pl.lag, pl.rows_per_tile, pl.width, pl.n_tiles);
+  return cudaGetLastError();
+}
+
+template <typename XT>
+static cudaError_t dispatch_narrow(const FusedPlan& pl, const void* X, const unsigned char* y, long long N, int p,
+                                   unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
+                                   double* z_out, cudaStream_t st) {
+#define HSP_NARROW_ARGS pl, X, y, N, p, seed, beta, ctl, partial, z_out, st
+#define HSP_NARROW_CASE(E_)                                                                   \
+  if (pl.chunks == E_) {                                                                      \
+    if constexpr (sizeof(XT) == 4) {                                                          \
+      if (pl.eta_mode == 2) return launch_narrow<XT, E_, 2>(HSP_NARROW_ARGS);                 \
+    }                                                                                         \
+    return launch_narrow<XT, E_, 0>(HSP_NARROW_ARGS);                                         \
+  }
+  HSP_NARROW_CASE(4)
+  HSP_NARROW_CASE(8)
+  HSP_NARROW_CASE(16)
+#undef HSP_NARROW_CASE
+#undef HSP_NARROW_ARGS
+  return cudaErrorInvalidValue;
+}
+
 FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X) {
   FusedPlan pl{};
   const size_t elem = dtype == kF32 ? 4 : 8;
@@ -616,6 +910,8 @@ FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X) 
       return pl;
     }
   }
+  if (force != 0 && env_int("HSP_FUSED_NARROW", 1) && narrow_plan(dtype, N, p, num_sms, X, &pl)) return pl;
+  pl = FusedPlan{};
   pl.variant = 0;
   pl.n_tiles = (N + kGenThreads - 1) / kGenThreads;
   long long grid = (long long)num_sms * 4;
@@ -668,7 +964,11 @@ static cudaError_t dispatch_tma(const FusedPlan& pl, const void* X, const unsign
 cudaError_t fused_pass_launch(const FusedPlan& pl, const void* X, int dtype, const unsigned char* y, long long N,
                               int p, unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                               double* z_out, cudaStream_t st) {
-  if (pl.variant != 1 && N < 0) return cudaSuccess;
+  if (pl.variant == 0 && N < 0) return cudaSuccess;
+  if (pl.variant == 2) {
+    return dtype == kF32 ? dispatch_narrow<float>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st)
+                         : dispatch_narrow<double>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);
+  }
   if (pl.variant == 1) {
     return dtype == kF32 ? dispatch_tma<float>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st)
                          : dispatch_tma<double>(pl, X, y, N, p, seed, beta, ctl, partial, z_out, st);

@@ -454,7 +454,9 @@ int hsp_get_plan(const hsp_state* s, int* fused_ctas, int* chol_ctas, int* overl
   return HSP_OK;
 }
 long long hsp_get_launch_count(const hsp_state* s) { return s ? s->launches : 0; }
-const char* hsp_fused_variant(const hsp_state* s) { return (s && s->plan.variant == 1) ? "tma" : "generic"; }
+const char* hsp_fused_variant(const hsp_state* s) {
+  return !s ? "generic" : s->plan.variant == 1 ? "tma" : s->plan.variant == 2 ? "tma-narrow" : "generic";
+}
 
 long long hsp_dbg_chol_trace(const hsp_state* s, long long* rows, long long capacity) {
   if (!s) return fail(HSP_EINVAL, "state is NULL");

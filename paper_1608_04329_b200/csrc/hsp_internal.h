@@ -22,7 +22,7 @@ struct Ctl {
 enum { kF32 = 0, kF64 = 1 };
 
 struct FusedPlan {
-  int variant;        // 0 = generic, 1 = tma
+  int variant;        // 0 = generic, 1 = tma (wide rows), 2 = tma-narrow (width = L lanes per row, chunks = EMAX)
   int grid, block;
   size_t smem;
   int rows_per_tile;  // R
