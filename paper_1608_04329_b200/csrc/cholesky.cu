@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(kCholThreads, 1)
 chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_inv2, Ctl* __restrict__ ctl,
                  double* __restrict__ L, double* __restrict__ W, double* __restrict__ Wt, double* __restrict__ ws,
                  int* __restrict__ flags, const CholTask* __restrict__ tasks, const int* __restrict__ list_off, int p,
-                 int nt, unsigned long long* __restrict__ trace) {
+                 int nt, unsigned long long* __restrict__ trace, double* __restrict__ Lt) {
   extern __shared__ __align__(16) double pool[];
   double* S = pool + kPoolDoubles;                   // 64 x TLD
   double* X = S + CT * TLD;                          // 64 x TLD
@@ -400,6 +400,8 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
         *reinterpret_cast<double2*>(L + g) = l;
         *reinterpret_cast<double2*>(W + g) = *reinterpret_cast<const double2*>(X + r * TLD + c);
         *reinterpret_cast<double2*>(Wt + g) = make_double2(X[c * TLD + r], X[(c + 1) * TLD + r]);
+        if (Lt != nullptr)   // L^T, used by the block back-substitution when only a block-diagonal inverse is built
+          *reinterpret_cast<double2*>(Lt + g) = make_double2(c >= r ? S[c * TLD + r] : 0.0, c + 1 >= r ? S[(c + 1) * TLD + r] : 0.0);
       }
       __threadfence();
       __syncthreads();
@@ -432,8 +434,11 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
         for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb)
-            *reinterpret_cast<double2*>(L + (size_t)(i * CT + f.row0 + mb * 8 + f.g) * P + j * CT + f.col0 + nb * 8 + 2 * f.t) =
-                make_double2(out[mb][nb][0], out[mb][nb][1]);
+          {
+            const int r = i * CT + f.row0 + mb * 8 + f.g, c = j * CT + f.col0 + nb * 8 + 2 * f.t;
+            *reinterpret_cast<double2*>(L + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
+            if (Lt != nullptr) { Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1]; }
+          }
         __threadfence();
         __syncthreads();
         if (tid == 0) st_release(&fL[(size_t)i * nt + j], 1);
@@ -566,6 +571,66 @@ beta_gemv2_kernel(const double* __restrict__ Wt, const double* tv, double* __res
   }
 }
 
+// ---- d2 with a block-diagonal inverse (p > 1280): block forward / backward substitution over super-blocks of
+// B = 64 sb rows,   r_I = g_I - sum_{J<I} L_IJ t'_J,  t'_I = W_II r_I;   s_I = t'_I + e_I - sum_{J>I} (L_JI)^T beta_J,
+// beta_I = Wt_II s_I  (L^T is stored by the Cholesky kernel as Lt, so every product reads rows).  One generic
+// row-range x column-range product, a warp per row, chained by programmatic dependent launch:
+//   out[row] = (in ? in[row] : 0) + (add_e ? e_row : 0) -/+ sum_{c in [lo(row), hi(row))} M[row][c] x[c]
+// tri = 0: columns [c0, c1);  1: [c0, end of the row's tile) (W);  2: [start of the row's tile, c1) (Wt).
+__global__ void __launch_bounds__(kGemvWarps * 32)
+blk_gemv_kernel(const double* __restrict__ M, int P, int row0, int nrows, int c0, int c1, int tri, const double* x,
+                const double* in, double* out, int subtract, int add_e, int p, unsigned long long seed,
+                const Ctl* __restrict__ ctl) {
+  pdl_trigger();
+  const int row = row0 + blockIdx.x * kGemvWarps + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  const bool live = row < row0 + nrows;
+  const double* w = M + (size_t)(live ? row : row0) * P;
+  int lo = c0, hi = c1;
+  if (tri == 1) hi = (row / CT + 1) * CT;
+  if (tri == 2) lo = (row / CT) * CT;
+  if (!live) hi = lo;
+  const int base0 = (lo / kGemvPass) * kGemvPass;
+  double2 wr[16];
+  gemv_load(wr, w, base0, lo, hi, lane);
+  double e = 0.0;
+  if (add_e && lane == 0 && live && row < p) {
+    const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
+    e = norm_inv(uniform_a(seed, (unsigned long long)row, sweep, TAG_E));
+  }
+  pdl_wait();
+  double s0 = 0.0, s1 = 0.0;
+  gemv_dot(wr, x, base0, lo, hi, lane, s0, s1);
+  for (int base = base0 + kGemvPass; base < hi; base += kGemvPass) {
+    gemv_load(wr, w, base, lo, hi, lane);
+    gemv_dot(wr, x, base, lo, hi, lane, s0, s1);
+  }
+  double s = s0 + s1;
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  if (lane == 0 && live) {
+    const double a = (in != nullptr ? __ldcg(in + row) : 0.0) + e;
+    out[row] = subtract ? a - s : a + s;
+  }
+}
+
+// finish of the block solve: status check, history append, k <- k + 1 (one CTA; after the last beta block)
+__global__ void __launch_bounds__(256)
+beta_finish_kernel(const double* beta, int p, Ctl* __restrict__ ctl) {
+  pdl_wait();
+  const unsigned long long k = ctl->sweep + 1ull;
+  double* __restrict__ h_beta = ctl->h_beta;
+  const unsigned long long hrow = k - 1ull - ctl->hist_base;
+  bool bad = false;
+  for (int j = threadIdx.x; j < p; j += blockDim.x) {
+    const double b = __ldcg(beta + j);
+    bad |= !isfinite(b);
+    if (h_beta != nullptr) h_beta[hrow * (unsigned long long)p + j] = b;
+  }
+  if (bad) atomicCAS(&ctl->status, 0, -5);
+  __syncthreads();
+  if (threadIdx.x == 0) ctl->sweep = k;
+}
+
 // FREEZE_BETA (tests): beta stays; append it to the history and advance the sweep counter.
 __global__ void __launch_bounds__(256)
 beta_keep_kernel(const double* __restrict__ beta, int p, Ctl* __restrict__ ctl) {
@@ -589,25 +654,33 @@ static int env_int2(const char* name, int dflt) {
 cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_estimate) {
   pl->p = p; pl->nt = chol_tiles(p); pl->P = chol_ld(p);
   const int nt = pl->nt;
+  // Inverse factor: the whole W = L^-1 for nt <= 20 (d2 is then two matrix-vector products); for larger p only the
+  // diagonal super-blocks of sb x sb tiles (the full inverse would double the flops) and d2 is a block substitution.
+  const int sb_env = env_int2("HSP_CHOL_SB", 0);
+  const int sb = sb_env > 0 ? std::min(sb_env, nt) : (nt <= 20 ? nt : 8);
+  pl->sb = sb;
   const long long tile_tasks = (long long)nt * nt;
   CholSchedule best;
   int k_env = env_int2("HSP_CHOL_CTAS", 0);
   if (k_env > num_sms) k_env = num_sms;
   if (k_env > 0) {
-    best = chol_build_schedule(nt, nt, (int)std::min<long long>(k_env, tile_tasks));
+    best = chol_build_schedule(nt, sb, (int)std::min<long long>(k_env, tile_tasks));
     pl->overlap = k_env < num_sms;
   } else {
-    const double budget_us = 0.85 * fused_ms_estimate * 1e3;
+    // the cost model is calibrated with the factor's working set in L2; when G, L, Lt (or W, Wt) do not fit beside
+    // the X stream (p >= ~1500) the tile loads of the overlapped branch go to HBM: measured ~1.3x at p = 2000
+    const double ws_mb = 3.0 * (double)pl->P * pl->P * 8.0 / 1e6;
+    const double budget_us = 0.85 * fused_ms_estimate * 1e3 / (ws_mb > 48.0 ? 1.3 : 1.0);
     const int cands[] = {2, 4, 6, 8, 10, 12, 16, 20, 24, 32, 40, 48};
     bool found = false;
     if (nt <= 40)
       for (int k : cands) {
         if (k > tile_tasks || k >= num_sms / 2) break;
-        CholSchedule s = chol_build_schedule(nt, nt, k);
+        CholSchedule s = chol_build_schedule(nt, sb, k);
         if (s.makespan_us <= budget_us) { best = std::move(s); found = true; break; }
       }
     pl->overlap = found;
-    if (!found) best = chol_build_schedule(nt, nt, (int)std::min<long long>(num_sms, tile_tasks));
+    if (!found) best = chol_build_schedule(nt, sb, (int)std::min<long long>(num_sms, tile_tasks));
   }
   pl->K = best.K; pl->n_slots = best.n_slots; pl->n_tasks = (int)best.tasks.size(); pl->est_us = best.makespan_us;
   pl->n_flags = 2 * (size_t)nt * nt + (size_t)std::max(1, best.n_slots);
@@ -636,14 +709,14 @@ void chol_plan_destroy(CholPlan* pl) {
 }
 
 cudaError_t cholesky_launch(const CholPlan& pl, const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W,
-                            double* Wt, cudaStream_t st, long long* launches) {
+                            double* Wt, double* Lt, cudaStream_t st, long long* launches) {
   cudaError_t e = cudaMemsetAsync(pl.d_flags, 0, pl.n_flags * sizeof(int), st);
   if (e != cudaSuccess) return e;
   int p = pl.p, nt = pl.nt;
   double* ws = pl.d_ws; int* flags = pl.d_flags; const CholTask* tasks = pl.d_tasks; const int* list_off = pl.d_list_off;
   unsigned long long* trace = pl.d_trace;
   void* args[] = {(void*)&G, (void*)&lam_inv2, (void*)&ctl, (void*)&L, (void*)&W, (void*)&Wt, (void*)&ws, (void*)&flags,
-                  (void*)&tasks, (void*)&list_off, (void*)&p, (void*)&nt, (void*)&trace};
+                  (void*)&tasks, (void*)&list_off, (void*)&p, (void*)&nt, (void*)&trace, (void*)&Lt};
   e = cudaLaunchCooperativeKernel((const void*)chol_task_kernel, dim3(pl.K), dim3(kCholThreads), args, kCholSmem, st);
   if (launches) ++*launches;
   return e;
@@ -669,6 +742,39 @@ cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g
   if (e != cudaSuccess) return e;
   e = launch_pdl(beta_gemv2_kernel, grid, kGemvWarps * 32, st, pdl, Wt, (const double*)tv, beta, p, P, ctl);
   if (launches) *launches += 2;
+  return e;
+}
+
+cudaError_t beta_block_solve_launch(const double* L, const double* Lt, const double* W, const double* Wt, const double* g,
+                                    double* tv, double* rv, double* beta, int p, int sb, unsigned long long seed, Ctl* ctl,
+                                    cudaStream_t st, long long* launches) {
+  const int P = chol_ld(p), B = sb * CT, nsb = (P + B - 1) / B;
+  static const bool pdl = env_int2("HSP_NO_PDL", 0) == 0;
+  const Ctl* cc = ctl;
+  cudaError_t e = cudaSuccess;
+  auto launch = [&](const double* M, int row0, int nrows, int c0, int c1, int tri, const double* x, const double* in,
+                    double* out, int subtract, int add_e) {
+    if (e != cudaSuccess) return;
+    e = launch_pdl(blk_gemv_kernel, (nrows + kGemvWarps - 1) / kGemvWarps, kGemvWarps * 32, st, pdl, M, P, row0, nrows, c0,
+                   c1, tri, x, in, out, subtract, add_e, p, seed, cc);
+    if (launches) ++*launches;
+  };
+  // forward: tv = L^-1 g
+  for (int I = 0; I < nsb; ++I) {
+    const int r0 = I * B, nr = std::min(B, P - r0);
+    const double* rhs = g;
+    if (I > 0) { launch(L, r0, nr, 0, r0, 0, tv, g, rv, 1, 0); rhs = rv; }       // r_I = g_I - L_{I,<I} t'_{<I}
+    launch(W, r0, nr, r0, r0 + nr, 1, rhs, nullptr, tv, 0, 0);                    // t'_I = W_II r_I
+  }
+  // backward: beta = L^-T (tv + e)
+  for (int I = nsb - 1; I >= 0; --I) {
+    const int r0 = I * B, nr = std::min(B, P - r0);
+    launch(Lt, r0, nr, r0 + nr, P, 0, beta, tv, rv, 1, 1);                        // s_I = t'_I + e_I - (L_{>I,I})^T beta_{>I}
+    launch(Wt, r0, nr, r0, r0 + nr, 2, rv, nullptr, beta, 0, 0);                  // beta_I = Wt_II s_I
+  }
+  if (e != cudaSuccess) return e;
+  e = launch_pdl(beta_finish_kernel, 1, 256, st, pdl, (const double*)beta, p, ctl);
+  if (launches) ++*launches;
   return e;
 }
 

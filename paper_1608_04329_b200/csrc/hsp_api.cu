@@ -36,7 +36,7 @@ struct hsp_state {
   cudaStream_t own_stream = nullptr;
   unsigned flags = 0; int num_sms = 0;
   void* own_X = nullptr; unsigned char* own_y = nullptr;
-  double *G = nullptr, *L = nullptr, *W = nullptr, *Wt = nullptr, *beta = nullptr, *lam_inv2 = nullptr,
+  double *G = nullptr, *L = nullptr, *Lt = nullptr, *rv = nullptr, *W = nullptr, *Wt = nullptr, *beta = nullptr, *lam_inv2 = nullptr,
          *nu_inv = nullptr, *g = nullptr, *tv = nullptr, *partial = nullptr, *z = nullptr, *mu = nullptr;
   int pd_ctas = 0;                   // CTAs (= partial rows) of the paper-design X^T z product
   CholPlan chol{};
@@ -61,7 +61,7 @@ static void free_state(hsp_state* s) {
   if (s->ev_join) cudaEventDestroy(s->ev_join);
   if (s->stream2) cudaStreamDestroy(s->stream2);
   if (s->own_stream) cudaStreamDestroy(s->own_stream);
-  void* ptrs[] = {s->own_X, s->own_y, s->G, s->L, s->W, s->Wt, s->beta, s->lam_inv2, s->nu_inv, s->g, s->tv, s->partial,
+  void* ptrs[] = {s->own_X, s->own_y, s->G, s->L, s->Lt, s->rv, s->W, s->Wt, s->beta, s->lam_inv2, s->nu_inv, s->g, s->tv, s->partial,
                   s->z, s->mu, s->side, s->ctl, s->h_beta, s->h_lambda, s->h_tau};
   for (void* q : ptrs) if (q) cudaFree(q);
   chol_plan_destroy(&s->chol);
@@ -94,7 +94,7 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
   auto side_branch = [&]() -> int {
     CK(scales_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, do_scales ? 0 : 1, B));
     *kernels += 1;
-    if (do_beta) CK(cholesky_launch(s->chol, s->G, s->lam_inv2, s->ctl, s->L, s->W, s->Wt, B, kernels));
+    if (do_beta) CK(cholesky_launch(s->chol, s->G, s->lam_inv2, s->ctl, s->L, s->W, s->Wt, s->Lt, B, kernels));
     return HSP_OK;
   };
   if (serial) { const int rc = side_branch(); if (rc) return rc; }
@@ -126,7 +126,9 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
     CK(reduce_partials_launch(s->partial, n_part, s->p, s->g, A));
     *kernels += 1;
   }
-  if (do_beta) CK(beta_solve_launch(s->W, s->Wt, s->g, s->tv, s->beta, s->p, s->seed, s->ctl, A, kernels));
+  if (do_beta && s->chol.sb < s->chol.nt)
+    CK(beta_block_solve_launch(s->L, s->Lt, s->W, s->Wt, s->g, s->tv, s->rv, s->beta, s->p, s->chol.sb, s->seed, s->ctl, A, kernels));
+  else if (do_beta) CK(beta_solve_launch(s->W, s->Wt, s->g, s->tv, s->beta, s->p, s->seed, s->ctl, A, kernels));
   else { CK(beta_keep_launch(s->beta, s->p, s->ctl, A)); *kernels += 1; }
   return HSP_OK;
 }
@@ -173,7 +175,8 @@ static int create_common(hsp_state** out, hsp_state* s) {
   const size_t pp = (size_t)p * p * sizeof(double), pv = (size_t)p * sizeof(double);
   const size_t P = (size_t)chol_ld(p), PP = P * P * sizeof(double), Pv = P * sizeof(double);
   CK(cudaMalloc(&s->G, pp)); CK(cudaMalloc(&s->L, PP)); CK(cudaMalloc(&s->W, PP)); CK(cudaMalloc(&s->Wt, PP));
-  CK(cudaMalloc(&s->beta, pv)); CK(cudaMalloc(&s->lam_inv2, pv)); CK(cudaMalloc(&s->nu_inv, pv));
+  CK(cudaMalloc(&s->beta, Pv));   // beta padded to P with zeros (the block solve reads whole tiles)
+  CK(cudaMalloc(&s->lam_inv2, pv)); CK(cudaMalloc(&s->nu_inv, pv));
   CK(cudaMalloc(&s->g, Pv)); CK(cudaMalloc(&s->tv, Pv));     // padded to P with zeros (the GEMVs read whole tiles)
   s->pd_ctas = paper_design_ctas(N, s->num_sms);
   CK(cudaMalloc(&s->partial, (size_t)std::max(s->plan.grid * s->plan.groups, s->pd_ctas) * pv));
@@ -191,7 +194,12 @@ static int create_common(hsp_state** out, hsp_state* s) {
   if (h_bad) return fail(HSP_EINVAL, "y must contain only 0 and 1");
   // cold start: beta = 0; lambda = nu = tau = xi = 1
   std::vector<double> ones((size_t)p, 1.0);
-  CK(cudaMemsetAsync(s->beta, 0, pv, s->stream));
+  CK(cudaMemsetAsync(s->beta, 0, Pv, s->stream));
+  if (s->chol.sb < s->chol.nt) {
+    CK(cudaMalloc(&s->Lt, PP)); CK(cudaMalloc(&s->rv, Pv));
+    CK(cudaMemsetAsync(s->Lt, 0, PP, s->stream)); CK(cudaMemsetAsync(s->rv, 0, Pv, s->stream));
+    CK(cudaMemsetAsync(s->W, 0, PP, s->stream)); CK(cudaMemsetAsync(s->Wt, 0, PP, s->stream));
+  }
   CK(cudaMemsetAsync(s->g, 0, Pv, s->stream));
   CK(cudaMemsetAsync(s->tv, 0, Pv, s->stream));
   CK(cudaMemsetAsync(s->L, 0, PP, s->stream));

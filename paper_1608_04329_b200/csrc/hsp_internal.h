@@ -69,6 +69,7 @@ CholSchedule chol_build_schedule(int nt, int sb_tiles, int K);
 
 struct CholPlan {
   int p = 0, nt = 0, P = 0, K = 0, n_slots = 0, n_tasks = 0;
+  int sb = 0;                        // tiles per inverse super-block (sb == nt: the whole inverse factor is built)
   bool overlap = false;              // the branch is expected to hide behind the fused pass on K SMs of its own
   double est_us = 0.0;
   CholTask* d_tasks = nullptr;
@@ -84,9 +85,13 @@ int chol_ld(int p);                    // P = 64 nt: leading dimension of L, W, 
 cudaError_t chol_plan_create(CholPlan* plan, int p, int num_sms, double fused_ms_estimate);
 void chol_plan_destroy(CholPlan* plan);
 cudaError_t cholesky_launch(const CholPlan& plan, const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W,
-                            double* Wt, cudaStream_t st, long long* launches);
+                            double* Wt, double* Lt, cudaStream_t st, long long* launches);
 cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g, double* tv, double* beta, int p,
                               unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches);
+// block substitution with a block-diagonal inverse (sb < nt); rv: scratch of P doubles
+cudaError_t beta_block_solve_launch(const double* L, const double* Lt, const double* W, const double* Wt, const double* g,
+                                    double* tv, double* rv, double* beta, int p, int sb, unsigned long long seed, Ctl* ctl,
+                                    cudaStream_t st, long long* launches);
 cudaError_t beta_keep_launch(const double* beta, int p, Ctl* ctl, cudaStream_t st);
 
 // ---- scale conditionals (e1, e2, e3) and draw output (g): scales.cu

@@ -187,3 +187,14 @@ def test_invalid_y_rejected():
     with pytest.raises(hsp.HspError) as ei:
         hsp.HorseshoeProbit(X, y, 1)
     assert ei.value.code == -1
+
+
+@pytest.mark.parametrize("sb,p,n_rows", [(2, 333, 3001), (1, 200, 2003), (3, 1000, 4001), (8, 2000, 6001)])
+def test_block_diagonal_inverse_and_block_substitution(sb, p, n_rows, monkeypatch):
+    """d2 by block forward/backward substitution with a block-diagonal inverse (the p > 1280 path), forced at
+    small p through HSP_CHOL_SB: the whole sweep against the oracle."""
+    monkeypatch.setenv("HSP_CHOL_SB", str(sb))
+    wl = hsp_synth.make("C3", "cuda", n_rows=n_rows, p=p)
+    X64 = wl.X.double()
+    w = run_parity(wl, 6, gram=(X64.T @ X64).cpu().numpy())
+    assert w["beta"] < 1e-5
