@@ -13,7 +13,7 @@ constexpr int kGK = 16;   // rows per smem chunk
 
 template <typename XT>
 __global__ void __launch_bounds__(256)
-gram_kernel(const XT* __restrict__ X, long long N, int p, double* __restrict__ out, int tiles_side,
+gram_kernel(const XT* __restrict__ X, long long N, int p, double* __restrict__ out, int slot0,
             long long rows_per_split) {
   __shared__ double As[kGK][kGT + 4];
   __shared__ double Bs[kGK][kGT + 4];
@@ -22,7 +22,7 @@ gram_kernel(const XT* __restrict__ X, long long N, int p, double* __restrict__ o
   while (t >= ti + 1) { t -= ti + 1; ++ti; }
   const int tj = t;
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-  const long long r_begin = (long long)blockIdx.y * rows_per_split;
+  const long long r_begin = (long long)(slot0 + blockIdx.y) * rows_per_split;     // slot q owns rows [q rps, (q+1) rps)
   const long long r_end = (r_begin + rows_per_split < N) ? r_begin + rows_per_split : N;
   double acc[4][4];
 #pragma unroll
@@ -53,7 +53,7 @@ gram_kernel(const XT* __restrict__ X, long long N, int p, double* __restrict__ o
     }
     __syncthreads();
   }
-  double* dst = out + (size_t)blockIdx.y * p * p;
+  double* dst = out + (size_t)(slot0 + blockIdx.y) * p * p;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const int a = ti * kGT + ty * 4 + i;
@@ -63,7 +63,6 @@ gram_kernel(const XT* __restrict__ X, long long N, int p, double* __restrict__ o
       if (a < p && b < p && b <= a) dst[(size_t)a * p + b] = acc[i][j];
     }
   }
-  (void)tiles_side;
 }
 
 __global__ void gram_reduce_kernel(const double* __restrict__ part, int splits, int p, double* __restrict__ G) {
@@ -83,33 +82,46 @@ __global__ void gram_mirror_kernel(double* __restrict__ G, int p) {
   if (b > a) G[idx] = G[(size_t)b * p + a];
 }
 
-int gram_splits(long long N, int p, int num_sms) {
+// Row partition of the Gram: `slots` equal row ranges (a multiple of 16 rows each), each accumulated on its own and
+// summed in slot order.  Enough slots to fill the SMs; and, for large X, at least 16 so that hsp_create_host can
+// overlap the upload of row chunk c+1 with the Gram of chunk c.  The partition depends only on (N, p, dtype, SMs):
+// the device and the host entry points give bit-identical G.
+GramPlan gram_plan(long long N, int p, int dtype, int num_sms) {
+  GramPlan g{};
   const int ts = (p + kGT - 1) / kGT;
   const long long tiles = (long long)ts * (ts + 1) / 2;
-  long long splits = (2LL * num_sms + tiles - 1) / tiles;
+  long long per_chunk = (2LL * num_sms + tiles - 1) / tiles;            // slots launched together
+  if (per_chunk > 64) per_chunk = 64;
+  const double x_bytes = (double)N * p * (dtype == kF32 ? 4.0 : 8.0);
+  long long chunks = (long long)(x_bytes / (128.0 * 1024 * 1024));
+  chunks = chunks < 1 ? 1 : chunks > 16 ? 16 : chunks;
+  long long slots = per_chunk * chunks;
   const long long max_by_rows = (N + 4095) / 4096;
-  if (splits > max_by_rows) splits = max_by_rows;
-  if (splits > 64) splits = 64;
-  if (splits < 1) splits = 1;
-  return (int)splits;
+  if (slots > max_by_rows) { slots = max_by_rows < 1 ? 1 : max_by_rows; chunks = 1; per_chunk = slots; }
+  g.slots = (int)slots; g.chunks = (int)chunks; g.slots_per_chunk = (int)per_chunk;
+  g.rows_per_slot = ((N + slots - 1) / slots + kGK - 1) / kGK * kGK;
+  return g;
 }
 
-// scratch: splits * p * p doubles (may alias G when splits == 1)
-cudaError_t gram_launch(const void* X, int dtype, long long N, int p, double* G, double* scratch, int splits,
-                        cudaStream_t st) {
+// Gram of the row chunk c (its slots_per_chunk slots) into scratch.
+cudaError_t gram_chunk_launch(const GramPlan& g, int chunk, const void* X, int dtype, long long N, int p, double* scratch,
+                              cudaStream_t st) {
   const int ts = (p + kGT - 1) / kGT;
   const int tiles = ts * (ts + 1) / 2;
-  const long long rps = ((N + splits - 1) / splits + kGK - 1) / kGK * kGK;
-  dim3 grid(tiles, splits);
+  dim3 grid(tiles, g.slots_per_chunk);
+  const int slot0 = chunk * g.slots_per_chunk;
   if (dtype == kF32)
-    gram_kernel<float><<<grid, 256, 0, st>>>(static_cast<const float*>(X), N, p, scratch, ts, rps);
+    gram_kernel<float><<<grid, 256, 0, st>>>(static_cast<const float*>(X), N, p, scratch, slot0, g.rows_per_slot);
   else
-    gram_kernel<double><<<grid, 256, 0, st>>>(static_cast<const double*>(X), N, p, scratch, ts, rps);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
+    gram_kernel<double><<<grid, 256, 0, st>>>(static_cast<const double*>(X), N, p, scratch, slot0, g.rows_per_slot);
+  return cudaGetLastError();
+}
+
+// G = sum of the slots in slot order, mirrored to the upper triangle.
+cudaError_t gram_finish_launch(const GramPlan& g, int p, const double* scratch, double* G, cudaStream_t st) {
   const size_t n = (size_t)p * p;
-  gram_reduce_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(scratch, splits, p, G);
-  e = cudaGetLastError();
+  gram_reduce_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(scratch, g.slots, p, G);
+  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   gram_mirror_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(G, p);
   return cudaGetLastError();

@@ -36,6 +36,7 @@ struct hsp_state {
   cudaStream_t own_stream = nullptr;
   unsigned flags = 0; int num_sms = 0;
   void* own_X = nullptr; unsigned char* own_y = nullptr;
+  const void* host_X = nullptr;      // hsp_create_host: X is uploaded in row chunks, overlapped with the Gram
   double *G = nullptr, *L = nullptr, *Lt = nullptr, *rv = nullptr, *W = nullptr, *Wt = nullptr, *beta = nullptr, *lam_inv2 = nullptr,
          *nu_inv = nullptr, *g = nullptr, *tv = nullptr, *partial = nullptr, *z = nullptr, *mu = nullptr;
   int pd_ctas = 0;                   // CTAs (= partial rows) of the paper-design X^T z product
@@ -45,6 +46,7 @@ struct hsp_state {
   double *h_beta = nullptr, *h_lambda = nullptr, *h_tau = nullptr;
   long long h_cap = 0, h_n = 0, host_sweep = 0;
   bool z_valid = false;
+  int* h_status = nullptr;           // pinned host word for the status read of hsp_get_draws
   FusedPlan plan{};
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   cudaGraphExec_t graph_exec = nullptr; unsigned graph_flags = ~0u; long long graph_kernels = 0;
@@ -65,6 +67,7 @@ static void free_state(hsp_state* s) {
                   s->z, s->mu, s->side, s->ctl, s->h_beta, s->h_lambda, s->h_tau};
   for (void* q : ptrs) if (q) cudaFree(q);
   chol_plan_destroy(&s->chol);
+  if (s->h_status) cudaFreeHost(s->h_status);
   delete s;
 }
 
@@ -181,6 +184,7 @@ static int create_common(hsp_state** out, hsp_state* s) {
   s->pd_ctas = paper_design_ctas(N, s->num_sms);
   CK(cudaMalloc(&s->partial, (size_t)std::max(s->plan.grid * s->plan.groups, s->pd_ctas) * pv));
   CK(cudaMalloc(&s->ctl, sizeof(Ctl)));
+  CK(cudaMallocHost(&s->h_status, sizeof(int)));
   // validate y in {0,1}
   int* bad = nullptr;
   CK(cudaMalloc(&bad, sizeof(int)));
@@ -209,14 +213,32 @@ static int create_common(hsp_state** out, hsp_state* s) {
   c.h_beta = c.h_lambda = c.h_tau = nullptr;
   CK(cudaMemcpyAsync(s->ctl, &c, sizeof(Ctl), cudaMemcpyHostToDevice, s->stream));
   CK(cudaStreamSynchronize(s->stream));   // `ones` and `c` are stack/heap temporaries
-  // c0: G = X^T X once
-  const int splits = gram_splits(N, p, s->num_sms);
+  // c0: G = X^T X once, by row chunks; with host input the upload of chunk c+1 (copy stream) runs
+  // beside the Gram of chunk c
+  const GramPlan gp = gram_plan(N, p, s->dtype, s->num_sms);
   double* scratch = s->W;                  // W (>= p*p doubles) is free until the first sweep
-  if (splits > 1) CK(cudaMalloc(&scratch, (size_t)splits * pp));
-  cudaError_t e = gram_launch(s->X, s->dtype, N, p, s->G, scratch, splits, s->stream);
-  s->launches += 3;
+  if (gp.slots > 1) CK(cudaMalloc(&scratch, (size_t)gp.slots * pp));
+  cudaError_t e = cudaSuccess;
+  const size_t row_bytes = (size_t)p * (s->dtype == HSP_F32 ? 4 : 8);
+  const long long chunk_rows = gp.rows_per_slot * gp.slots_per_chunk;
+  for (int c = 0; c < gp.chunks && e == cudaSuccess; ++c) {
+    if (s->host_X != nullptr) {
+      const long long r0 = (long long)c * chunk_rows;
+      const long long r1 = (c == gp.chunks - 1) ? N : std::min(N, r0 + chunk_rows);
+      if (r1 > r0) {
+        e = cudaMemcpyAsync(static_cast<char*>(s->own_X) + (size_t)r0 * row_bytes,
+                            static_cast<const char*>(s->host_X) + (size_t)r0 * row_bytes, (size_t)(r1 - r0) * row_bytes,
+                            cudaMemcpyHostToDevice, s->stream2);
+        if (e == cudaSuccess) e = cudaEventRecord(s->ev_fork, s->stream2);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s->stream, s->ev_fork, 0);
+      }
+    }
+    if (e == cudaSuccess) e = gram_chunk_launch(gp, c, s->X, s->dtype, N, p, scratch, s->stream);
+  }
+  if (e == cudaSuccess) e = gram_finish_launch(gp, p, scratch, s->G, s->stream);
+  s->launches += gp.chunks + 2;
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
-  if (splits > 1) cudaFree(scratch);
+  if (gp.slots > 1) cudaFree(scratch);
   if (e != cudaSuccess) return cuda_fail(e, "gram");
   *out = s;
   return HSP_OK;
@@ -266,10 +288,9 @@ int hsp_create_host(hsp_state** out, const void* X_host, int x_dtype, const unsi
   const size_t xb = (size_t)N * p * (x_dtype == HSP_F32 ? 4 : 8);
   cudaError_t e = cudaMalloc(&s->own_X, xb);
   if (e == cudaSuccess) e = cudaMalloc(&s->own_y, (size_t)N);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(s->own_X, X_host, xb, cudaMemcpyHostToDevice, s->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(s->own_y, y_host, (size_t)N, cudaMemcpyHostToDevice, s->stream);
-  if (e != cudaSuccess) { const int rc = cuda_fail(e, "upload of X, y"); free_state(s); return rc; }
-  s->X = s->own_X; s->y = s->own_y;
+  if (e != cudaSuccess) { const int rc = cuda_fail(e, "allocation / upload of y"); free_state(s); return rc; }
+  s->X = s->own_X; s->y = s->own_y; s->host_X = X_host;   // X itself is uploaded chunk by chunk in create_common
   const int rc = create_common(out, s);
   if (rc != HSP_OK) { free_state(s); *out = nullptr; }
   return rc;
@@ -313,12 +334,9 @@ int hsp_sweep(hsp_state* s, long long n_iter) {
   }
   s->h_n = n_iter;
   if (n_iter == 0) return HSP_OK;
-  // history window of this call: only these fields of Ctl are touched from the host
-  struct { unsigned long long hist_base; } hb{(unsigned long long)s->host_sweep};
-  CK(cudaMemcpyAsync(reinterpret_cast<char*>(s->ctl) + offsetof(Ctl, hist_base), &hb, sizeof(hb), cudaMemcpyHostToDevice, s->stream));
-  double* hp[3] = {s->h_beta, s->h_lambda, s->h_tau};
-  CK(cudaMemcpyAsync(reinterpret_cast<char*>(s->ctl) + offsetof(Ctl, h_beta), hp, sizeof(hp), cudaMemcpyHostToDevice, s->stream));
-  CK(cudaStreamSynchronize(s->stream));   // hb / hp are stack temporaries
+  // history window of this call: set by a one-thread kernel (its arguments are copied at launch: no host sync)
+  CK(set_history_launch(s->ctl, (unsigned long long)s->host_sweep, s->h_beta, s->h_lambda, s->h_tau, s->stream));
+  s->launches += 1;
   if (s->flags & HSP_STORE_Z) s->z_valid = !(s->flags & HSP_FREEZE_Z) || s->z_valid;
   else if (!(s->flags & HSP_FREEZE_Z)) s->z_valid = false;
   if (s->flags & HSP_NO_GRAPH) {
@@ -357,14 +375,19 @@ int hsp_sync(const hsp_state* s) {
 
 int hsp_get_draws(const hsp_state* s, double* beta, double* lambda, double* tau) {
   if (!s) return fail(HSP_EINVAL, "state is NULL");
-  const int rc = sync_status(s);
+  // status and draws are copied on the stream and the stream is synchronised once
   const size_t np = (size_t)s->h_n * s->p * sizeof(double);
+  int* st = s->h_status;
+  CK(cudaMemcpyAsync(st, reinterpret_cast<const char*>(s->ctl) + offsetof(Ctl, status), sizeof(int), cudaMemcpyDeviceToHost, s->stream));
   if (s->h_n > 0) {
-    if (beta) CK(cudaMemcpy(beta, s->h_beta, np, cudaMemcpyDefault));
-    if (lambda) CK(cudaMemcpy(lambda, s->h_lambda, np, cudaMemcpyDefault));
-    if (tau) CK(cudaMemcpy(tau, s->h_tau, (size_t)s->h_n * sizeof(double), cudaMemcpyDefault));
+    if (beta) CK(cudaMemcpyAsync(beta, s->h_beta, np, cudaMemcpyDefault, s->stream));
+    if (lambda) CK(cudaMemcpyAsync(lambda, s->h_lambda, np, cudaMemcpyDefault, s->stream));
+    if (tau) CK(cudaMemcpyAsync(tau, s->h_tau, (size_t)s->h_n * sizeof(double), cudaMemcpyDefault, s->stream));
   }
-  return rc;
+  CK(cudaStreamSynchronize(s->stream));
+  if (*st == HSP_ENOTPD) return fail(HSP_ENOTPD, "Cholesky breakdown: Q is not positive definite");
+  if (*st == HSP_ENUMERIC) return fail(HSP_ENUMERIC, "non-finite value in the chain state");
+  return HSP_OK;
 }
 
 int hsp_get_latent(const hsp_state* s, double* z, signed char* side) {

@@ -49,9 +49,11 @@ cudaError_t paper_design_launch(const void* X, int dtype, const unsigned char* y
                                 int num_sms, cudaStream_t st);
 
 // ---- Gram (c0): gram.cu
-cudaError_t gram_launch(const void* X, int dtype, long long N, int p, double* G, double* scratch, int splits,
-                        cudaStream_t st);
-int gram_splits(long long N, int p, int num_sms);
+struct GramPlan { int slots, chunks, slots_per_chunk; long long rows_per_slot; };
+GramPlan gram_plan(long long N, int p, int dtype, int num_sms);
+cudaError_t gram_chunk_launch(const GramPlan& g, int chunk, const void* X, int dtype, long long N, int p, double* scratch,
+                              cudaStream_t st);
+cudaError_t gram_finish_launch(const GramPlan& g, int p, const double* scratch, double* G, cudaStream_t st);
 
 // ---- Q build (c), Cholesky + inverse factor (d1), beta draw (d2): cholesky.cu, chol_schedule.cu
 // One tile task of the Cholesky task graph (64x64 tiles).  type 0: tile L(i,j), i >= j; type 1: inverse tile
@@ -97,6 +99,7 @@ cudaError_t beta_keep_launch(const double* beta, int p, Ctl* ctl, cudaStream_t s
 // ---- scale conditionals (e1, e2, e3) and draw output (g): scales.cu
 cudaError_t scales_launch(const double* beta, double* lam_inv2, double* nu_inv, Ctl* ctl, int p, unsigned long long seed,
                           int freeze_scales, cudaStream_t st);
+cudaError_t set_history_launch(Ctl* ctl, unsigned long long hist_base, double* hb, double* hl, double* ht, cudaStream_t st);
 cudaError_t validate_y_launch(const unsigned char* y, long long N, int* bad, cudaStream_t st);
 cudaError_t side_launch(const unsigned char* y, long long N, signed char* side, cudaStream_t st);
 

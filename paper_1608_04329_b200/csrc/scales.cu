@@ -67,6 +67,10 @@ scales_kernel(const double* __restrict__ beta, double* __restrict__ lam_inv2, do
   if (bad) atomicCAS(&ctl->status, 0, -5);
 }
 
+__global__ void set_history_kernel(Ctl* ctl, unsigned long long hist_base, double* hb, double* hl, double* ht) {
+  ctl->hist_base = hist_base; ctl->h_beta = hb; ctl->h_lambda = hl; ctl->h_tau = ht;
+}
+
 __global__ void validate_y_kernel(const unsigned char* __restrict__ y, long long N, int* __restrict__ bad) {
   const long long stride = (long long)gridDim.x * blockDim.x;
   bool b = false;
@@ -83,6 +87,11 @@ __global__ void side_kernel(const unsigned char* __restrict__ y, long long N, si
 cudaError_t scales_launch(const double* beta, double* lam_inv2, double* nu_inv, Ctl* ctl, int p, unsigned long long seed,
                           int freeze_scales, cudaStream_t st) {
   scales_kernel<<<1, kScaleThreads, 0, st>>>(beta, lam_inv2, nu_inv, ctl, p, seed, freeze_scales);
+  return cudaGetLastError();
+}
+
+cudaError_t set_history_launch(Ctl* ctl, unsigned long long hist_base, double* hb, double* hl, double* ht, cudaStream_t st) {
+  set_history_kernel<<<1, 1, 0, st>>>(ctl, hist_base, hb, hl, ht);
   return cudaGetLastError();
 }
 
