@@ -139,6 +139,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--paper-design", action="store_true", help="A/B: rows a1-a3 by the paper's own decomposition (two X reads, rejection sampler)")
+    ap.add_argument("--sharded", action="store_true", help="N > 1: ONE chain, rows of X sharded over the ranks, one NCCL all-reduce of p doubles per sweep (strong scaling)")
     ap.add_argument("--graph", action="store_true", help="replay the captured CUDA graph in the timed region (no per-kernel events)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -163,16 +164,31 @@ def main():
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    elif args.sharded:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29533")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
 
     # Multi-GPU: independent chains, one per GPU, same data recipe, seed + rank.
     wl = hsp_synth.make(args.workload, dev)
     seed = multi.chain_seed(wl.seed, rank)
     stream = torch.cuda.Stream(device=dev)
     x_bytes = wl.X.numel() * wl.X.element_size()
+    if args.sharded:
+        seed = wl.seed                                 # one chain: every rank uses the same Philox key
+        r0, r1 = multi.shard_rows(wl.N, rank, world)
+        Xl, yl = wl.X[r0:r1].contiguous(), wl.y[r0:r1].contiguous()
+        x_bytes = Xl.numel() * Xl.element_size()
     with torch.cuda.stream(stream):
-        chain = hsp.HorseshoeProbit(wl.X, wl.y, seed, stream=stream)
-        chain.set_flags((0 if args.graph else hsp.HSP_NO_GRAPH) | (hsp.HSP_PAPER_DESIGN if args.paper_design else 0))
-        chain.sweep(args.warmup)
+        if args.sharded:
+            chain = hsp.HorseshoeProbit(Xl, yl, seed, stream=stream, row_offset=r0)
+            chain.set_flags(hsp.HSP_NO_GRAPH)
+            multi.sharded_init(chain)
+            run_sweeps = lambda n: multi.sharded_sweeps(chain, n)
+        else:
+            chain = hsp.HorseshoeProbit(wl.X, wl.y, seed, stream=stream)
+            chain.set_flags((0 if args.graph else hsp.HSP_NO_GRAPH) | (hsp.HSP_PAPER_DESIGN if args.paper_design else 0))
+            run_sweeps = chain.sweep
+        run_sweeps(args.warmup)
         chain.sync()
         chain.fused_pass_ms()                     # reset the event accumulator
         k0 = chain.launch_count()
@@ -182,7 +198,7 @@ def main():
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         with ClockSampler(local_rank) as clocks:
             ev0.record(stream)
-            chain.sweep(args.steps)
+            run_sweeps(args.steps)
             ev1.record(stream)
             chain.sync()
             torch.cuda.synchronize(dev)
@@ -197,12 +213,12 @@ def main():
         b, lam, tau = chain.get_draws()
         assert np.all(np.isfinite(b)) and np.all(np.isfinite(lam)) and np.all(tau > 0)
     ms = multi.max_over_ranks(ms, dev)
-    value = multi.whole_job_rate(args.steps, ms)
+    value = multi.whole_job_rate(args.steps, ms) if not args.sharded else args.steps / (ms * 1e-3)
 
     line = None
     if rank == 0:
         peaks, peak_kind = measured_peaks()
-        alg_bytes = x_bytes + wl.N            # X once + y; z is not stored in the timed run
+        alg_bytes = x_bytes + (wl.N if not args.sharded else (r1 - r0))   # X once + y; z is not stored in the timed run
         roofline = None
         if fused_n > 0 and fused_ms > 0:
             achieved = alg_bytes / (fused_ms * 1e-3) / 1e9
@@ -217,7 +233,8 @@ def main():
                         "alg_bytes_per_launch": alg_bytes, "avg_launch_ms": fused_ms, "launches_timed": fused_n,
                         "share_of_step": fused_ms / (ms / args.steps)}
         line = {"metric": "gibbs_sweeps_per_sec", "value": value, "unit": "sweeps/s", "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "strong" if args.sharded else "weak",
                 "vs_baseline": value / PAPER_SWEEPS_PER_S if args.workload == "C3" else None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": WORKLOAD_DESC[args.workload], "x_dtype": str(wl.X.dtype).replace("torch.", ""),
@@ -225,12 +242,13 @@ def main():
                            "l2": "X (%.1f GB) is larger than L2 and is streamed once per step" % (x_bytes / 1e9)
                            if x_bytes > 256e6 else "inputs fit L2: latency-bound config, absolute number only",
                            "launch_mode": "cuda-graph replay" if args.graph else "direct launches, 2 streams",
-                           "multi_gpu": "independent chains, seed+rank, no collective" if world > 1 else "single chain",
+                           "multi_gpu": ("one chain, rows sharded over %d ranks, one all-reduce of p doubles per sweep" % world) if args.sharded
+                           else "independent chains, seed+rank, no collective" if world > 1 else "single chain",
                            "vs_baseline_note": "paper: 83.3 sweeps/s on a Titan X, fp32 (PAPER.md:305); context, not the target"},
                 "clocks": clocks.summary(), "gpu_launches": int(launches), "roofline": roofline}
 
     # ---- e2e: host buffers through the C-ABI, uploads and per-sweep readback inside the timed region
-    if not args.no_e2e:
+    if not args.no_e2e and not args.sharded:
         Xh = wl.X.cpu().pin_memory()
         yh = wl.y.cpu().pin_memory()
         e2e_steps = args.steps
@@ -260,7 +278,7 @@ def main():
                                    "the one-off upload is amortised over the steps" % e2e_steps}
 
     # ---- cpu_baseline: the oracle on a bounded row sample, rank 0, single GPU run only
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.sharded:
         n_s = min(wl.N, 60000)
         Xs = wl.X[:n_s].cpu().numpy()
         ys = wl.y[:n_s].cpu().numpy()
@@ -270,7 +288,7 @@ def main():
                                           f"p-only work as measured; {wall:.1f} s of CPU); host has {os.cpu_count()} cores"}
     if rank == 0:
         print(json.dumps(line), flush=True)
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
 
 

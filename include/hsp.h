@@ -74,6 +74,25 @@ int hsp_create(hsp_state** out, const void* X, int x_dtype, const unsigned char*
 int hsp_create_host(hsp_state** out, const void* X_host, int x_dtype, const unsigned char* y_host,
                     long long N, int p, unsigned long long seed, void* stream);
 
+/* Row-sharded chains (the z_i are conditionally independent, so the rows of
+ * X split across GPUs).  Each rank creates a chain on ITS rows; row_offset = global index of its first row, so
+ * that the Philox counter of z_i is the global row and the draws do not depend on the number of ranks.  After
+ * create, the caller sums hsp_gram_device (p*p doubles) over the ranks, in place, once.  Then, per sweep:
+ *   hsp_sweep_begin   enqueues a1-a3, b on the local rows (-> hsp_xtz_device, p doubles) and e1-e3, c, d1
+ *   <caller>          sums hsp_xtz_device over the ranks in place (one all-reduce of p doubles, e.g. NCCL on the
+ *                     same stream); every rank then holds the same X^T z bit for bit
+ *   hsp_sweep_end     enqueues d2: every rank draws the same beta (same counters, same inputs)
+ * hsp_sweep_prepare(n) reserves the history for the next n begin/end pairs (what hsp_get_draws returns).
+ * All asynchronous on the stream; no host synchronisation per sweep.  X, y DEVICE, borrowed, as in hsp_create.
+ * Errors as hsp_create / hsp_sweep; HSP_EINVAL if the calls are made out of order.                  */
+int hsp_create_shard(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N_local,
+                     int p, unsigned long long seed, long long row_offset, void* stream);
+int hsp_sweep_prepare(hsp_state* s, long long n_iter);
+int hsp_sweep_begin(hsp_state* s);
+int hsp_sweep_end(hsp_state* s);
+double* hsp_xtz_device(hsp_state* s);   /* DEVICE, p doubles, owned by the library   */
+double* hsp_gram_device(hsp_state* s);  /* DEVICE, p*p doubles row-major (symmetric) */
+
 /* Run n_iter sweeps (steps a1..g above, in the order PAPER.md:188-189 fixes), asynchronously on the
  * stream.  The draws of this call replace the history of the previous call.  n_iter >= 0.
  * Errors: HSP_EINVAL, HSP_ENOMEM (history n_iter*(2p+1)*8 bytes), HSP_ECUDA.  A Cholesky breakdown

@@ -46,6 +46,14 @@ def lib():
     L.hsp_create.argtypes = [C.POINTER(vp), vp, C.c_int, vp, ll, C.c_int, ull, vp]
     L.hsp_create_host.argtypes = [C.POINTER(vp), vp, C.c_int, vp, ll, C.c_int, ull, vp]
     L.hsp_sweep.argtypes = [vp, ll]
+    L.hsp_create_shard.argtypes = [C.POINTER(vp), vp, C.c_int, vp, ll, C.c_int, ull, ll, vp]
+    L.hsp_sweep_prepare.argtypes = [vp, ll]
+    L.hsp_sweep_begin.argtypes = [vp]
+    L.hsp_sweep_end.argtypes = [vp]
+    L.hsp_xtz_device.argtypes = [vp]
+    L.hsp_xtz_device.restype = vp
+    L.hsp_gram_device.argtypes = [vp]
+    L.hsp_gram_device.restype = vp
     L.hsp_get_draws.argtypes = [vp, vp, vp, vp]
     L.hsp_sync.argtypes = [vp]
     L.hsp_destroy.argtypes = [vp]
@@ -93,7 +101,7 @@ def _stream_handle(stream):
 class HorseshoeProbit:
     """hsp_create / hsp_sweep / hsp_get_draws on torch CUDA tensors (or host arrays with host=True)."""
 
-    def __init__(self, X, y, seed, stream=None, host=False):
+    def __init__(self, X, y, seed, stream=None, host=False, row_offset=None):
         import torch
         L = lib()
         self._h = C.c_void_p()
@@ -111,7 +119,11 @@ class HorseshoeProbit:
             assert X.is_cuda and y.is_cuda and X.is_contiguous() and y.is_contiguous() and y.dtype == torch.uint8
             dt = {torch.float32: HSP_F32, torch.float64: HSP_F64}[X.dtype]
             self._keep = (X, y)                       # borrowed by the library: keep alive
-            _check(L.hsp_create(C.byref(self._h), X.data_ptr(), dt, y.data_ptr(), self.N, self.p, seed, sh))
+            if row_offset is None:
+                _check(L.hsp_create(C.byref(self._h), X.data_ptr(), dt, y.data_ptr(), self.N, self.p, seed, sh))
+            else:
+                _check(L.hsp_create_shard(C.byref(self._h), X.data_ptr(), dt, y.data_ptr(), self.N, self.p, seed,
+                                          int(row_offset), sh))
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
@@ -133,6 +145,30 @@ class HorseshoeProbit:
 
     def sync(self):
         _check(lib().hsp_sync(self._h))
+
+    # ---- row-sharded chains: hsp_sweep_prepare / _begin / _end and the two buffers the caller all-reduces
+    def sweep_prepare(self, n_iter):
+        _check(lib().hsp_sweep_prepare(self._h, n_iter))
+        self.n_last = n_iter
+
+    def sweep_begin(self):
+        _check(lib().hsp_sweep_begin(self._h))
+
+    def sweep_end(self):
+        _check(lib().hsp_sweep_end(self._h))
+
+    def _device_view(self, ptr, shape):
+        import torch
+
+        class _Mem:                                   # zero-copy view of library memory (CUDA array interface)
+            __cuda_array_interface__ = {"shape": shape, "typestr": "<f8", "data": (int(ptr), False), "version": 3}
+        return torch.as_tensor(_Mem(), device=self._keep[0].device)
+
+    def xtz_tensor(self):
+        return self._device_view(lib().hsp_xtz_device(self._h), (self.p,))
+
+    def gram_tensor(self):
+        return self._device_view(lib().hsp_gram_device(self._h), (self.p, self.p))
 
     def get_draws(self, out=None):
         """(beta[n,p], lambda[n,p], tau[n]) of the last sweep() call as numpy arrays, or into the

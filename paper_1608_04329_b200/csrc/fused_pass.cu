@@ -220,7 +220,7 @@ template <typename XT, int RT, int C, int W, int EM>
 __global__ void __launch_bounds__(kTmaThreads, 1)
 fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
                unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
-               double* __restrict__ partial, double* __restrict__ z_out, int S, int D, long long n_tiles) {
+               double* __restrict__ partial, double* __restrict__ z_out, int S, int D, long long n_tiles, long long row_off) {
   constexpr int V = Vec<XT>::V;
   using Acc = typename Vec<XT>::Acc;
   constexpr bool kF32 = sizeof(XT) == 4;
@@ -302,7 +302,7 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         const bool valid = (lane < RT) && (i < N);
         const int y3 = load_y(n + 3LL * ns);
         // the Philox uniform does not depend on eta either: compute it before waiting
-        const double u = uniform_a(seed, (unsigned long long)(valid ? i : 0), sweep, TAG_Z);
+        const double u = uniform_a(seed, (unsigned long long)(row_off + (valid ? i : 0)), sweep, TAG_Z);
         const double ystar = 2.0 * (double)y0 - 1.0;
         mbar_wait(&eta_full[st], ph);
         double eta = 0.0;
@@ -501,7 +501,7 @@ __global__ void __launch_bounds__(kNarrowThreads, 1)
 fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
                   unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
                   double* __restrict__ partial, double* __restrict__ z_out, int S, int D, int RT, int L,
-                  long long n_tiles) {
+                  long long n_tiles, long long row_off) {
   constexpr bool kF32 = sizeof(XT) == 4;
   using Acc = typename std::conditional<kF32, float, double>::type;
   extern __shared__ __align__(128) unsigned char smem[];
@@ -578,7 +578,7 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
           const long long i = row0 + b + lane;
           const bool valid = i < N;
           const int yi = valid ? (int)y[i] : 1;
-          const double u = uniform_a(seed, (unsigned long long)(valid ? i : 0), sweep, TAG_Z);
+          const double u = uniform_a(seed, (unsigned long long)(row_off + (valid ? i : 0)), sweep, TAG_Z);
           const double ystar = 2.0 * (double)yi - 1.0;
           if (!waited) { mbar_wait(&eta_full[st], ph); waited = true; }
           const double eta = eta_s[st * RT + b + lane];
@@ -691,7 +691,7 @@ template <typename XT>
 __global__ void __launch_bounds__(kGenThreads)
 fused_pass_generic(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
                    unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
-                   double* __restrict__ partial, double* __restrict__ z_out, int csg /*pow2 column slots*/) {
+                   double* __restrict__ partial, double* __restrict__ z_out, int csg /*pow2 column slots*/, long long row_off) {
   __shared__ double z_s[kGenThreads];
   __shared__ double red[kGenThreads];
   const int tid = threadIdx.x;
@@ -715,7 +715,7 @@ fused_pass_generic(const XT* __restrict__ X, const unsigned char* __restrict__ y
       double eta = 0.0;
       for (int j = 0; j < p; ++j) eta = fma((double)xr[j], beta[j], eta);
       const double ystar = 2.0 * (double)y[i] - 1.0;
-      const double u = uniform_a(seed, (unsigned long long)i, sweep, TAG_Z);
+      const double u = uniform_a(seed, (unsigned long long)(row_off + i), sweep, TAG_Z);
       z = ystar * tnpos(ystar * eta, u);
       if (z_out != nullptr) z_out[i] = z;
     }
@@ -850,7 +850,7 @@ static cudaError_t launch_narrow(const FusedPlan& pl, const void* X, const unsig
   }
   if (N < 0) return cudaSuccess;
   kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
-                                          pl.stages, pl.lag, pl.rows_per_tile, pl.width, pl.n_tiles);
+                                          pl.stages, pl.lag, pl.rows_per_tile, pl.width, pl.n_tiles, pl.row_offset);
   return cudaGetLastError();
 }
 
@@ -934,7 +934,7 @@ static cudaError_t launch_tma(const FusedPlan& pl, const void* X, const unsigned
   }
   if (N < 0) return cudaSuccess;     // prepare-only call (sets the attribute outside stream capture)
   kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
-                                          pl.stages, pl.lag, pl.n_tiles);
+                                          pl.stages, pl.lag, pl.n_tiles, pl.row_offset);
   return cudaGetLastError();
 }
 
@@ -977,10 +977,10 @@ cudaError_t fused_pass_launch(const FusedPlan& pl, const void* X, int dtype, con
   while (csg < p && csg < kGenThreads) csg <<= 1;
   if (dtype == kF32)
     fused_pass_generic<float><<<pl.grid, pl.block, 0, st>>>(static_cast<const float*>(X), y, N, p, seed, beta, ctl,
-                                                            partial, z_out, csg);
+                                                            partial, z_out, csg, pl.row_offset);
   else
     fused_pass_generic<double><<<pl.grid, pl.block, 0, st>>>(static_cast<const double*>(X), y, N, p, seed, beta, ctl,
-                                                             partial, z_out, csg);
+                                                             partial, z_out, csg, pl.row_offset);
   return cudaGetLastError();
 }
 

@@ -19,6 +19,7 @@
 using namespace hsp;
 
 static thread_local std::string g_err;
+static thread_local long long g_pending_row_offset = 0;   // hsp_create_shard -> hsp_create
 static int fail(int code, const std::string& msg) { g_err = msg; return code; }
 static int cuda_fail(cudaError_t e, const char* what) {
   g_err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -32,6 +33,7 @@ static int cuda_fail(cudaError_t e, const char* what) {
 
 struct hsp_state {
   const void* X = nullptr; int dtype = 0; const unsigned char* y = nullptr; long long N = 0; int p = 0;
+  long long row_offset = 0;          // global index of local row 0 (hsp_create_shard)
   unsigned long long seed = 0; cudaStream_t stream = nullptr; cudaStream_t stream2 = nullptr;
   cudaStream_t own_stream = nullptr;
   unsigned flags = 0; int num_sms = 0;
@@ -46,6 +48,7 @@ struct hsp_state {
   double *h_beta = nullptr, *h_lambda = nullptr, *h_tau = nullptr;
   long long h_cap = 0, h_n = 0, host_sweep = 0;
   bool z_valid = false;
+  long long split_left = 0; bool split_open = false;   // hsp_sweep_prepare / _begin / _end
   int* h_status = nullptr;           // pinned host word for the status read of hsp_get_draws
   FusedPlan plan{};
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
@@ -54,6 +57,8 @@ struct hsp_state {
   std::vector<cudaEvent_t> tev;   // event pairs around the fused pass (direct-launch mode)
   size_t tev_used = 0; double fused_ms_sum = 0.0; long long fused_n = 0;
 };
+
+static int prepare_history(hsp_state* s, long long n_iter);
 
 static void free_state(hsp_state* s) {
   if (!s) return;
@@ -84,16 +89,19 @@ static int drain_fused_events(hsp_state* s) {
 // Enqueue one sweep.  `timed`: bracket the fused pass with CUDA events (direct-launch mode only).
 //   stream A:  fused pass (a1-a3) ------------------------------> [join] reduce (b) -> d2 (two products; k <- k+1)
 //   stream B:  scales (e1, e2, e3; lambda, tau history) -> Q build + Cholesky + inverse factor (c, d1)
-static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
+// phases: 1 = up to and including the reduction of X^T z (and the whole side branch), 2 = the beta draw, 3 = both.
+static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels, int phases = 3) {
   cudaStream_t A = s->stream;
   const bool serial = (s->flags & HSP_SERIAL) != 0;
   cudaStream_t B = serial ? A : s->stream2;
   const bool do_z = !(s->flags & HSP_FREEZE_Z), do_scales = !(s->flags & HSP_FREEZE_SCALES),
              do_beta = !(s->flags & HSP_FREEZE_BETA);
+  if (phases == 2) goto draw;
   if (!serial) {
     CK(cudaEventRecord(s->ev_fork, A));
     CK(cudaStreamWaitEvent(B, s->ev_fork, 0));
   }
+  {
   auto side_branch = [&]() -> int {
     CK(scales_launch(s->beta, s->lam_inv2, s->nu_inv, s->ctl, s->p, s->seed, do_scales ? 0 : 1, B));
     *kernels += 1;
@@ -129,6 +137,9 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels) {
     CK(reduce_partials_launch(s->partial, n_part, s->p, s->g, A));
     *kernels += 1;
   }
+  }
+  if (phases == 1) return HSP_OK;
+draw:
   if (do_beta && s->chol.sb < s->chol.nt)
     CK(beta_block_solve_launch(s->L, s->Lt, s->W, s->Wt, s->g, s->tv, s->rv, s->beta, s->p, s->chol.sb, s->seed, s->ctl, A, kernels));
   else if (do_beta) CK(beta_solve_launch(s->W, s->Wt, s->g, s->tv, s->beta, s->p, s->seed, s->ctl, A, kernels));
@@ -173,6 +184,7 @@ static int create_common(hsp_state** out, hsp_state* s) {
   CK(chol_plan_create(&s->chol, p, s->num_sms, fused_ms_est));
   const int fused_sms = s->chol.overlap ? s->num_sms - s->chol.K : s->num_sms;
   s->plan = fused_plan(s->dtype, N, p, fused_sms, s->X);
+  s->plan.row_offset = s->row_offset;
   // set opt-in shared-memory attributes now, outside any stream capture
   CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, -1, p, 0, nullptr, nullptr, nullptr, nullptr, s->stream));
   const size_t pp = (size_t)p * p * sizeof(double), pv = (size_t)p * sizeof(double);
@@ -244,6 +256,25 @@ static int create_common(hsp_state** out, hsp_state* s) {
   return HSP_OK;
 }
 
+static int prepare_history(hsp_state* s, long long n_iter) {
+  const int p = s->p;
+  if (n_iter > s->h_cap) {
+    CK(cudaStreamSynchronize(s->stream));
+    if (s->h_beta) { cudaFree(s->h_beta); cudaFree(s->h_lambda); cudaFree(s->h_tau); s->h_beta = s->h_lambda = s->h_tau = nullptr; }
+    s->h_cap = 0;
+    CK(cudaMalloc(&s->h_beta, (size_t)n_iter * p * sizeof(double)));
+    CK(cudaMalloc(&s->h_lambda, (size_t)n_iter * p * sizeof(double)));
+    CK(cudaMalloc(&s->h_tau, (size_t)n_iter * sizeof(double)));
+    s->h_cap = n_iter;
+  }
+  s->h_n = n_iter;
+  if (n_iter == 0) return HSP_OK;
+  // history window of this call: set by a one-thread kernel (its arguments are copied at launch: no host sync)
+  CK(set_history_launch(s->ctl, (unsigned long long)s->host_sweep, s->h_beta, s->h_lambda, s->h_tau, s->stream));
+  s->launches += 1;
+  return HSP_OK;
+}
+
 extern "C" {
 
 const char* hsp_last_error(void) { return g_err.c_str(); }
@@ -269,6 +300,7 @@ int hsp_create(hsp_state** out, const void* X, int x_dtype, const unsigned char*
   hsp_state* s = new (std::nothrow) hsp_state();
   if (!s) return fail(HSP_ENOMEM, "out of host memory");
   s->X = X; s->dtype = x_dtype; s->y = y; s->N = N; s->p = p; s->seed = seed; s->stream = (cudaStream_t)stream;
+  s->row_offset = g_pending_row_offset;
   const int rc = create_common(out, s);
   if (rc != HSP_OK) { free_state(s); *out = nullptr; }
   return rc;
@@ -296,6 +328,49 @@ int hsp_create_host(hsp_state** out, const void* X_host, int x_dtype, const unsi
   return rc;
 }
 
+int hsp_create_shard(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N_local, int p,
+                     unsigned long long seed, long long row_offset, void* stream) {
+  if (row_offset < 0) { if (out) *out = nullptr; return fail(HSP_EINVAL, "row_offset must be >= 0"); }
+  // same validation as hsp_create; the offset must be known before the plan is made
+  g_pending_row_offset = row_offset;
+  const int rc = hsp_create(out, X, x_dtype, y, N_local, p, seed, stream);
+  g_pending_row_offset = 0;
+  return rc;
+}
+
+int hsp_sweep_prepare(hsp_state* s, long long n_iter) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  if (n_iter < 0) return fail(HSP_EINVAL, "n_iter must be >= 0");
+  if (s->flags & HSP_PAPER_DESIGN) return fail(HSP_EINVAL, "HSP_PAPER_DESIGN is not available for sharded sweeps");
+  s->split_left = n_iter; s->split_open = false;
+  return prepare_history(s, n_iter);
+}
+
+int hsp_sweep_begin(hsp_state* s) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  if (s->split_left <= 0 || s->split_open) return fail(HSP_EINVAL, "hsp_sweep_begin: call hsp_sweep_prepare first / finish the open sweep");
+  if (s->flags & HSP_STORE_Z) s->z_valid = !(s->flags & HSP_FREEZE_Z) || s->z_valid;
+  else if (!(s->flags & HSP_FREEZE_Z)) s->z_valid = false;
+  long long k = 0;
+  const int rc = enqueue_sweep(s, (s->flags & HSP_NO_GRAPH) != 0, &k, 1);
+  if (rc != HSP_OK) return rc;
+  s->launches += k; s->split_open = true;
+  return HSP_OK;
+}
+
+int hsp_sweep_end(hsp_state* s) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  if (!s->split_open) return fail(HSP_EINVAL, "hsp_sweep_end without hsp_sweep_begin");
+  long long k = 0;
+  const int rc = enqueue_sweep(s, false, &k, 2);
+  if (rc != HSP_OK) return rc;
+  s->launches += k; s->split_open = false; s->split_left -= 1; s->host_sweep += 1;
+  return HSP_OK;
+}
+
+double* hsp_xtz_device(hsp_state* s) { return s ? s->g : nullptr; }
+double* hsp_gram_device(hsp_state* s) { return s ? s->G : nullptr; }
+
 int hsp_destroy(hsp_state* s) {
   if (!s) return HSP_OK;
   cudaStreamSynchronize(s->stream);
@@ -322,21 +397,8 @@ int hsp_set_flags(hsp_state* s, unsigned flags) {
 int hsp_sweep(hsp_state* s, long long n_iter) {
   if (!s) return fail(HSP_EINVAL, "state is NULL");
   if (n_iter < 0) return fail(HSP_EINVAL, "n_iter must be >= 0");
-  const int p = s->p;
-  if (n_iter > s->h_cap) {
-    CK(cudaStreamSynchronize(s->stream));
-    if (s->h_beta) { cudaFree(s->h_beta); cudaFree(s->h_lambda); cudaFree(s->h_tau); s->h_beta = s->h_lambda = s->h_tau = nullptr; }
-    s->h_cap = 0;
-    CK(cudaMalloc(&s->h_beta, (size_t)n_iter * p * sizeof(double)));
-    CK(cudaMalloc(&s->h_lambda, (size_t)n_iter * p * sizeof(double)));
-    CK(cudaMalloc(&s->h_tau, (size_t)n_iter * sizeof(double)));
-    s->h_cap = n_iter;
-  }
-  s->h_n = n_iter;
+  { const int rc = prepare_history(s, n_iter); if (rc != HSP_OK) return rc; }
   if (n_iter == 0) return HSP_OK;
-  // history window of this call: set by a one-thread kernel (its arguments are copied at launch: no host sync)
-  CK(set_history_launch(s->ctl, (unsigned long long)s->host_sweep, s->h_beta, s->h_lambda, s->h_tau, s->stream));
-  s->launches += 1;
   if (s->flags & HSP_STORE_Z) s->z_valid = !(s->flags & HSP_FREEZE_Z) || s->z_valid;
   else if (!(s->flags & HSP_FREEZE_Z)) s->z_valid = false;
   if (s->flags & HSP_NO_GRAPH) {

@@ -33,6 +33,7 @@ struct FusedPlan {
   int groups;         // G: row groups of compute warps (partial rows = grid * G)
   int eta_mode;       // EM: arithmetic of the eta phase for fp32 X (fused_pass.cu)
   long long n_tiles;
+  long long row_offset;   // global index of local row 0 (row-sharded chains: the Philox counter of z_i is the GLOBAL row)
 };
 
 // ---- fused pass (a1-a3) and reduce (b): fused_pass.cu

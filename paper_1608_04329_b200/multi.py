@@ -53,3 +53,33 @@ def split_rhat(chains):
     B = h * means.var(dim=0, unbiased=True)
     var_plus = (h - 1) / h * W + B / h
     return torch.sqrt(var_plus / W)
+
+
+# ---- row-sharded chain (include/hsp.h "Row-sharded chains"): the driver loop, on any chain object that offers
+# sweep_prepare(n) / sweep_begin() / sweep_end(), xtz_tensor() and gram_tensor() (HorseshoeProbit created with
+# row_offset=...; the CPU tests drive an oracle-backed stand-in through the same loop).
+
+def shard_rows(N, rank, world_size):
+    """Rows [r0, r1) of rank `rank`: contiguous, sizes differ by at most one row."""
+    base, rem = divmod(int(N), int(world_size))
+    r0 = rank * base + min(rank, rem)
+    return r0, r0 + base + (1 if rank < rem else 0)
+
+
+def sharded_init(chain, group=None):
+    """Sum the per-shard Gram matrices in place, once (p*p doubles)."""
+    if world()[1] > 1:
+        dist.all_reduce(chain.gram_tensor(), op=dist.ReduceOp.SUM, group=group)
+
+
+def sharded_sweeps(chain, n_iter, group=None):
+    """n_iter sweeps of a row-sharded chain: per sweep one all-reduce of X^T z (p doubles) between the local pass
+    and the beta draw.  Everything is enqueued on the current stream; there is no host synchronisation."""
+    chain.sweep_prepare(n_iter)
+    g = chain.xtz_tensor()
+    ws = world()[1]
+    for _ in range(n_iter):
+        chain.sweep_begin()
+        if ws > 1:
+            dist.all_reduce(g, op=dist.ReduceOp.SUM, group=group)
+        chain.sweep_end()
