@@ -86,11 +86,14 @@ __global__ void gram_mirror_kernel(double* __restrict__ G, int p) {
 // summed in slot order.  Enough slots to fill the SMs; and, for large X, at least 16 so that hsp_create_host can
 // overlap the upload of row chunk c+1 with the Gram of chunk c.  The partition depends only on (N, p, dtype, SMs):
 // the device and the host entry points give bit-identical G.
-GramPlan gram_plan(long long N, int p, int dtype, int num_sms) {
+GramPlan gram_plan(long long N, int p, int dtype, int num_sms, bool tensor_core) {
   GramPlan g{};
-  const int ts = (p + kGT - 1) / kGT;
+  g.tensor_core = tensor_core;
+  const int tile = tensor_core ? 128 : kGT;
+  const int ts = (p + tile - 1) / tile;
   const long long tiles = (long long)ts * (ts + 1) / 2;
   long long per_chunk = (2LL * num_sms + tiles - 1) / tiles;            // slots launched together
+  if (tensor_core) per_chunk = tiles <= num_sms ? num_sms / tiles : 1;   // one CTA per SM (TMEM, 128 registers x 512): one wave
   if (per_chunk > 64) per_chunk = 64;
   const double x_bytes = (double)N * p * (dtype == kF32 ? 4.0 : 8.0);
   long long chunks = (long long)(x_bytes / (128.0 * 1024 * 1024));

@@ -8,6 +8,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <string>
 #include <vector>
 #include <algorithm>
@@ -48,6 +49,7 @@ struct hsp_state {
   double *h_beta = nullptr, *h_lambda = nullptr, *h_tau = nullptr;
   long long h_cap = 0, h_n = 0, host_sweep = 0;
   bool z_valid = false;
+  bool gram_tc = false;              // the Gram was computed on the tensor cores (gram_tc.cu)
   long long split_left = 0; bool split_open = false;   // hsp_sweep_prepare / _begin / _end
   int* h_status = nullptr;           // pinned host word for the status read of hsp_get_draws
   FusedPlan plan{};
@@ -227,7 +229,12 @@ static int create_common(hsp_state** out, hsp_state* s) {
   CK(cudaStreamSynchronize(s->stream));   // `ones` and `c` are stack/heap temporaries
   // c0: G = X^T X once, by row chunks; with host input the upload of chunk c+1 (copy stream) runs
   // beside the Gram of chunk c
-  const GramPlan gp = gram_plan(N, p, s->dtype, s->num_sms);
+  // fp32 X and a large contraction: tcgen05 tensor cores (split-bf16 products, fp64 flush; ~1e-7 relative);
+  // otherwise exact fp64 DFMA tiles.  HSP_GRAM_TC = 0 / 1 forces the choice.
+  const char* tc_env = getenv("HSP_GRAM_TC");
+  const bool use_tc = s->dtype == HSP_F32 && ((tc_env && *tc_env) ? atoi(tc_env) != 0 : (double)N * p * p >= 2e10);
+  s->gram_tc = use_tc;
+  const GramPlan gp = gram_plan(N, p, s->dtype, s->num_sms, use_tc);
   double* scratch = s->W;                  // W (>= p*p doubles) is free until the first sweep
   if (gp.slots > 1) CK(cudaMalloc(&scratch, (size_t)gp.slots * pp));
   cudaError_t e = cudaSuccess;
@@ -245,7 +252,9 @@ static int create_common(hsp_state** out, hsp_state* s) {
         if (e == cudaSuccess) e = cudaStreamWaitEvent(s->stream, s->ev_fork, 0);
       }
     }
-    if (e == cudaSuccess) e = gram_chunk_launch(gp, c, s->X, s->dtype, N, p, scratch, s->stream);
+    if (e == cudaSuccess)
+      e = use_tc ? gram_tc_chunk_launch(gp, c, static_cast<const float*>(s->X), N, p, scratch, s->stream)
+                 : gram_chunk_launch(gp, c, s->X, s->dtype, N, p, scratch, s->stream);
   }
   if (e == cudaSuccess) e = gram_finish_launch(gp, p, scratch, s->G, s->stream);
   s->launches += gp.chunks + 2;

@@ -50,8 +50,10 @@ cudaError_t paper_design_launch(const void* X, int dtype, const unsigned char* y
                                 int num_sms, cudaStream_t st);
 
 // ---- Gram (c0): gram.cu
-struct GramPlan { int slots, chunks, slots_per_chunk; long long rows_per_slot; };
-GramPlan gram_plan(long long N, int p, int dtype, int num_sms);
+struct GramPlan { int slots, chunks, slots_per_chunk; long long rows_per_slot; bool tensor_core; };
+GramPlan gram_plan(long long N, int p, int dtype, int num_sms, bool tensor_core);
+// fp32 X on the tcgen05 tensor cores (split-bf16, fp64 flush): gram_tc.cu
+cudaError_t gram_tc_chunk_launch(const GramPlan& g, int chunk, const float* X, long long N, int p, double* scratch, cudaStream_t st);
 cudaError_t gram_chunk_launch(const GramPlan& g, int chunk, const void* X, int dtype, long long N, int p, double* scratch,
                               cudaStream_t st);
 cudaError_t gram_finish_launch(const GramPlan& g, int p, const double* scratch, double* G, cudaStream_t st);

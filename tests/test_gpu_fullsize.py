@@ -6,6 +6,7 @@ One whole sweep is checked against the oracle's definitions evaluated at full si
   a2  z_i = s_i TNpos(s_i eta_i, U_A(i, k, Z))   oracle.uniforms_many / oracle.tnpos_many, every row
   a3+b g = X^T z                 fp64 library product on the host from the ORACLE's z
   e1-e3 scale conditionals       the oracle chain itself (its scale step does not touch X)
+  c0 G = X^T X                   fp64 library product (the tensor-core Gram is within 1e-6 of it)
   c, d1, d2  Q = G + diag, L, beta   oracle.cholesky_lower / solve_lower (numpy.linalg.cholesky for p = 4000)
 No expected value comes from the CUDA path: the oracle side starts from the chain state read BEFORE the sweep.
 Tolerances: north_star's 1e-4 for fp32 X in the mixed metric of DESIGN.md R12 (observed values are printed);
@@ -117,5 +118,7 @@ def test_full_size_sweep_against_oracle(name, warm):
     print(f"{name} full size N={N} p={p} sweep {k} plan {plan}: z {ez:.3e}  X^Tz {eg:.3e}  beta {eb:.3e}  gram {e_gram:.3e}  "
           f"lam {e_lam:.3e} nu {e_nu:.3e} tau {e_tau:.3e} xi {e_xi:.3e}")
     assert ez <= 1e-4 and eg <= 1e-4 and eb <= 1e-4
-    assert e_gram <= 1e-12
+    # C3-C5 are above the size where create uses the tensor-core Gram (fp32 X, N p^2 >= 2e10): split-bf16 products with
+    # a truncating fp32 TMEM accumulation over <= 128 rows -> relative bias ~2e-7; exact DFMA path: 1e-13
+    assert e_gram <= 1e-6
     assert max(e_lam, e_nu, e_tau, e_xi) <= 1e-9

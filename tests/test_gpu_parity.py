@@ -198,3 +198,23 @@ def test_block_diagonal_inverse_and_block_substitution(sb, p, n_rows, monkeypatc
     X64 = wl.X.double()
     w = run_parity(wl, 6, gram=(X64.T @ X64).cpu().numpy())
     assert w["beta"] < 1e-5
+
+
+@pytest.mark.parametrize("name,n,p", [("C3", 5003, 333), ("C3", 3001, 1000), ("C4", 7001, 520), ("C3", 257, 128), ("C5", 2100, 2000)])
+def test_tensor_core_gram_matches_fp64_definition(name, n, p, monkeypatch):
+    """Row c0 on tcgen05 (split-bf16 products, fp32 TMEM accumulation over <= 128 rows, fp64 flush), forced at
+    small sizes: against the fp64 definition G = X^T X (library matmul).  The TMEM accumulation truncates: the
+    error is a relative bias of about -2e-7; bound 1e-6 of max|G|."""
+    monkeypatch.setenv("HSP_GRAM_TC", "1")
+    wl = hsp_synth.make(name, "cuda", n_rows=n, p=p)
+    X64 = wl.X.double()
+    Go = (X64.T @ X64).cpu().numpy()
+    g = hsp.HorseshoeProbit(wl.X, wl.y, 1)
+    Gg = g.get_gram()
+    g.close()
+    assert np.array_equal(Gg, Gg.T)
+    err = np.max(np.abs(Gg - Go)) / np.max(np.abs(Go))
+    print(name, n, p, "tensor-core Gram: max|dG|/max|G| =", err)
+    assert err <= 1e-6
+    # and the whole chain on top of it stays inside the fp32-X tolerance
+    run_parity(hsp_synth.make(name, "cuda", n_rows=n, p=p), 4, gram=Go)
