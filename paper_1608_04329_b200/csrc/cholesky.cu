@@ -679,8 +679,23 @@ cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_e
         CholSchedule s = chol_build_schedule(nt, sb, k);
         if (s.makespan_us <= budget_us) { best = std::move(s); found = true; break; }
       }
+    if (!found) {
+      // nothing hides completely.  A small branch (small p: C1, C2) is still better run BESIDE the pass on a few SMs
+      // than before it on all of them: compare  max(pass on the remaining SMs, 1.25 x branch on K)  with the serial sum.
+      const int k_all = (int)std::min<long long>(num_sms, tile_tasks);
+      CholSchedule serial = chol_build_schedule(nt, sb, k_all);
+      const double fused_us = fused_ms_estimate * 1e3;
+      double best_t = fused_us + serial.makespan_us;
+      if (nt <= 8)
+        for (int k : {1, 2, 4, 6, 8}) {
+          if (k > tile_tasks || k >= num_sms / 2) break;
+          CholSchedule s = chol_build_schedule(nt, sb, k);
+          const double t = std::max(fused_us * num_sms / (num_sms - k), 1.25 * s.makespan_us);
+          if (t < best_t) { best_t = t; best = std::move(s); found = true; }
+        }
+      if (!found) best = std::move(serial);
+    }
     pl->overlap = found;
-    if (!found) best = chol_build_schedule(nt, sb, (int)std::min<long long>(num_sms, tile_tasks));
   }
   pl->K = best.K; pl->n_slots = best.n_slots; pl->n_tasks = (int)best.tasks.size(); pl->est_us = best.makespan_us;
   pl->n_flags = 2 * (size_t)nt * nt + (size_t)std::max(1, best.n_slots);
