@@ -809,7 +809,7 @@ static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* 
   while (L < 32 && (p + L - 1) / L > 4) L <<= 1;
   const int E = (p + L - 1) / L;
   if (E > 16) return false;
-  int RT = (int)(32768 / row_bytes) / 32 * 32;
+  int RT = (int)(56000 / row_bytes) / 32 * 32;      // ~50 KB stages (4 fit): the per-tile overhead is what limits narrow rows
   RT = RT < 32 ? 32 : RT > 256 ? 256 : RT;
   if (env_int("HSP_NARROW_RT", 0) > 0) RT = env_int("HSP_NARROW_RT", 0) / 32 * 32;
   const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
@@ -821,7 +821,7 @@ static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* 
   }
   if (S < 3 || NarrowSmemLayout(S, RT, p, stage_bytes).total > budget) return false;
   int D = env_int("HSP_FUSED_LAG", 0);
-  if (D <= 0) D = (S - 1) / 2;
+  if (D <= 0) D = (S - 1) / 2 > 2 ? (S - 1) / 2 : 2;
   if (D > S - 2) D = S - 2;
   if (D < 1) D = 1;
   pl->variant = 2;
