@@ -28,6 +28,7 @@ WORKLOAD_DESC = {
     "C3": "C3 paper scale: N=1000000, p=1000, fp32 X iid N(0,1) (4 GB), fp64 state, 20 nonzeros, seed 3",
     "C4": "C4 correlated wide: N=250000, p=4000, fp32 AR(1) rows + intercept, 40 nonzeros, seed 4",
     "C5": "C5 large imbalanced: N=2000000, p=2000, fp32 X iid N(0,1) (16 GB), intercept -2, 50 nonzeros, seed 5",
+    "R1": "R1 shape of the paper's real-data run (PAPER.md:309): N=1295848, p=141, fp32, ~0.5 % positives, synthetic, seed 6",
 }
 
 

@@ -45,6 +45,9 @@ CONFIGS = {
     "C4": dict(N=250_000, p=4000, dtype=torch.float32, seed=4, sweeps=500),
     "C5": dict(N=2_000_000, p=2000, dtype=torch.float32, seed=5, sweeps=300),
     "C5b": dict(N=2_000_000, p=2000, dtype=torch.float32, seed=5, sweeps=300),
+    # stand-in for the SHAPE of the paper's real-data run (N = 1,295,848, p = 141, ybar = 0.0048;
+    # the clinical data itself is not available): iid N(0,1) columns + intercept, rare positives
+    "R1": dict(N=1_295_848, p=141, dtype=torch.float32, seed=6, sweeps=1000),
 }
 
 
@@ -54,12 +57,14 @@ def _planted_beta(name, p, rng):
         beta[:3] = [2.0, -1.5, 1.0]
         return beta
     nnz, lo, hi, first = {"C2": (10, 0.5, 2.0, 0), "C3": (20, 0.5, 2.0, 0), "C4": (40, 0.25, 1.5, 1),
-                          "C5": (50, 0.5, 2.0, 1), "C5b": (50, 0.5, 2.0, 1)}[name]
+                          "C5": (50, 0.5, 2.0, 1), "C5b": (50, 0.5, 2.0, 1), "R1": (10, 0.2, 0.6, 1)}[name]
     nnz = min(nnz, p - first)
     idx = first + rng.choice(p - first, size=nnz, replace=False)
     beta[idx] = rng.uniform(lo, hi, size=nnz) * rng.choice([-1.0, 1.0], size=nnz)
     if name == "C5":
         beta[0] = -2.0           # literal BASELINE.json reading (R15)
+    if name == "R1":
+        beta[0] = -2.59 * np.sqrt(1.0 + float(np.sum(beta ** 2)))    # Phi(-2.59) = 0.0048
     if name == "C5b":
         beta[0] = -1.645 * np.sqrt(1.0 + float(np.sum(beta ** 2)))   # gives ~5 % positives
     return beta
@@ -94,7 +99,7 @@ def make(name, device="cpu", n_rows=None, p=None):
             s = 0.75 ** 0.5
             for j in range(2, p):
                 blk[:, j] = 0.5 * blk[:, j - 1] + s * e[:, j]
-        elif name in ("C5", "C5b"):
+        elif name in ("C5", "C5b", "R1"):
             blk[:, 0] = 1.0
         X[r0:r1] = blk
         eps = torch.randn(r1 - r0, dtype=torch.float64, device=dev, generator=gen)

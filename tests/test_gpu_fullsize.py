@@ -49,7 +49,7 @@ def gram_fp64(X):
     return G.cpu().numpy()
 
 
-@pytest.mark.parametrize("name,warm", [("C3", 3), ("C4", 2), ("C5", 2)])
+@pytest.mark.parametrize("name,warm", [("C3", 3), ("C4", 2), ("C5", 2), ("R1", 12)])
 def test_full_size_sweep_against_oracle(name, warm):
     wl = hsp_synth.make(name, "cuda")
     N, p, seed = wl.N, wl.p, wl.seed
@@ -67,7 +67,7 @@ def test_full_size_sweep_against_oracle(name, warm):
     variant = g.fused_variant()
     Gg = g.get_gram()
     g.close()
-    assert variant == "tma"
+    assert variant == ("tma-narrow" if name == "R1" else "tma")
 
     # ---- a1, a2: every row
     y = wl.y.cpu().numpy()
