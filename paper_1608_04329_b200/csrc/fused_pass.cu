@@ -492,6 +492,12 @@ struct NarrowSmemLayout {
   }
 };
 
+// A stage is RT rows plus 1 KB that TMA never writes and that stays zero: the eta phase reads up to EMAX L - p
+// elements past the end of a row (times beta = 0), which for the last row of a tile lands in this pad.
+__host__ __device__ constexpr size_t narrow_stage_bytes(int RT, size_t row_bytes) {
+  return (((size_t)RT * row_bytes + 127) & ~(size_t)127) + 1024;
+}
+
 template <typename XT> __device__ __forceinline__ XT ld_shared_x(uint32_t a);
 template <> __device__ __forceinline__ float ld_shared_x<float>(uint32_t a) { return ld_shared_f32(a); }
 template <> __device__ __forceinline__ double ld_shared_x<double>(uint32_t a) { return ld_shared_f64(a); }
@@ -506,7 +512,7 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
   using Acc = typename std::conditional<kF32, float, double>::type;
   extern __shared__ __align__(128) unsigned char smem[];
   const size_t row_bytes = (size_t)p * sizeof(XT);
-  const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
+  const size_t stage_bytes = narrow_stage_bytes(RT, row_bytes);
   const NarrowSmemLayout lay(S, RT, p, stage_bytes);
   unsigned char* tiles = smem + lay.tiles;
   double* eta_s = reinterpret_cast<double*>(smem + lay.eta);
@@ -610,6 +616,8 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
     const int NG = kComputeThreadsAll / p > 0 ? kComputeThreadsAll / p : 1;   // p <= 512 here
     const int xg = tid / p, xj = tid - xg * p;
     const bool xz_on = xg < NG;
+    const int RPG = ((RT + NG - 1) / NG + 3) / 4 * 4;                      // rows of a tile per row group, a multiple of 4
+    const uint32_t z32a = smem_u32(z32), z64a = smem_u32(z64);
     double acc64 = 0.0;
     Acc acc = (Acc)0;
     const uint32_t rb = (uint32_t)row_bytes, sb = (uint32_t)stage_bytes;
@@ -628,16 +636,14 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
           if constexpr (kF32 && EM != 0) {
             float c = 0.f;
 #pragma unroll
-            for (int e = 0; e < EMAX; ++e)
-              if (l + e * L < p) c = fmaf(ld_shared_f32(xa + (uint32_t)(e * L) * 4u), bf[e], c);
+            for (int e = 0; e < EMAX; ++e) c = fmaf(ld_shared_f32(xa + (uint32_t)(e * L) * 4u), bf[e], c);   // past p: beta = 0
 #pragma unroll 1
             for (int off = L >> 1; off >= 1; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
             s = (double)c;
           } else {
             s = 0.0;
 #pragma unroll
-            for (int e = 0; e < EMAX; ++e)
-              if (l + e * L < p) s = fma((double)ld_shared_x<XT>(xa + (uint32_t)(e * L) * (uint32_t)sizeof(XT)), bd[e], s);
+            for (int e = 0; e < EMAX; ++e) s = fma((double)ld_shared_x<XT>(xa + (uint32_t)(e * L) * (uint32_t)sizeof(XT)), bd[e], s);
 #pragma unroll 1
             for (int off = L >> 1; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
           }
@@ -650,22 +656,32 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
       if (it >= D) {
         mbar_wait_a(zf0 + 8u * st_g, ph_g);
         if (xz_on) {
+          // rows [xg RPG, (xg+1) RPG) of the tile, four at a time (z as one 16-byte / two 16-byte loads)
           const uint32_t xa = tiles0 + st_g * sb + (uint32_t)xj * (uint32_t)sizeof(XT);
+          const int r_hi = (xg + 1) * RPG < RT ? (xg + 1) * RPG : RT;
           if constexpr (kF32) {
-            const float* zp = z32 + st_g * RT;
-#pragma unroll 4
-            for (int r = xg; r < RT; r += NG) acc = fmaf(ld_shared_f32(xa + (uint32_t)r * rb), zp[r], acc);
+            const uint32_t za = z32a + (uint32_t)(st_g * RT) * 4u;
+            for (int r = xg * RPG; r < r_hi; r += 4) {
+              const float4 z4 = ld_shared_f32x4(za + (uint32_t)r * 4u);
+              const uint32_t x0 = xa + (uint32_t)r * rb;
+              const float a0 = ld_shared_f32(x0), a1 = ld_shared_f32(x0 + rb), a2 = ld_shared_f32(x0 + 2u * rb), a3 = ld_shared_f32(x0 + 3u * rb);
+              acc = fmaf(a0, z4.x, acc); acc = fmaf(a1, z4.y, acc); acc = fmaf(a2, z4.z, acc); acc = fmaf(a3, z4.w, acc);
+            }
           } else {
-            const double* zp = z64 + st_g * RT;
-#pragma unroll 4
-            for (int r = xg; r < RT; r += NG) acc = fma(ld_shared_f64(xa + (uint32_t)r * rb), zp[r], acc);
+            const uint32_t za = z64a + (uint32_t)(st_g * RT) * 8u;
+            for (int r = xg * RPG; r < r_hi; r += 4) {
+              const double2 za01 = ld_shared_f64x2(za + (uint32_t)r * 8u), za23 = ld_shared_f64x2(za + (uint32_t)r * 8u + 16u);
+              const uint32_t x0 = xa + (uint32_t)r * rb;
+              const double a0 = ld_shared_f64(x0), a1 = ld_shared_f64(x0 + rb), a2 = ld_shared_f64(x0 + 2u * rb), a3 = ld_shared_f64(x0 + 3u * rb);
+              acc = fma(a0, za01.x, acc); acc = fma(a1, za01.y, acc); acc = fma(a2, za23.x, acc); acc = fma(a3, za23.y, acc);
+            }
           }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive_a(empty0 + 8u * st_g);
         if (++st_g == (uint32_t)S) { st_g = 0; ph_g ^= 1u; }
         if constexpr (kF32) {
-          rows_since_flush += (RT + NG - 1) / NG;
+          rows_since_flush += RPG;
           if (rows_since_flush >= kFlushRows) { rows_since_flush = 0; acc64 += (double)acc; acc = 0.f; }
         }
       }
@@ -812,7 +828,7 @@ static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* 
   int RT = (int)(56000 / row_bytes) / 32 * 32;      // ~50 KB stages (4 fit): the per-tile overhead is what limits narrow rows
   RT = RT < 32 ? 32 : RT > 256 ? 256 : RT;
   if (env_int("HSP_NARROW_RT", 0) > 0) RT = env_int("HSP_NARROW_RT", 0) / 32 * 32;
-  const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
+  const size_t stage_bytes = narrow_stage_bytes(RT, row_bytes);
   const size_t budget = 227 * 1024;
   int S = env_int("HSP_FUSED_STAGES", 0);
   if (S <= 0) {
@@ -825,7 +841,7 @@ static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* 
   if (D > S - 2) D = S - 2;
   if (D < 1) D = 1;
   pl->variant = 2;
-  pl->rows_per_tile = RT; pl->chunks = E <= 4 ? 4 : E <= 8 ? 8 : 16; pl->width = L; pl->stages = S; pl->lag = D;
+  pl->rows_per_tile = RT; pl->chunks = E <= 4 ? 4 : E <= 6 ? 6 : E <= 8 ? 8 : E <= 12 ? 12 : 16; pl->width = L; pl->stages = S; pl->lag = D;
   pl->groups = 1;
   int em = dtype == kF32 ? env_int("HSP_FUSED_ETA", 2) : 0;
   pl->eta_mode = (em == 0) ? 0 : 2;
@@ -867,7 +883,9 @@ static cudaError_t dispatch_narrow(const FusedPlan& pl, const void* X, const uns
     return launch_narrow<XT, E_, 0>(HSP_NARROW_ARGS);                                         \
   }
   HSP_NARROW_CASE(4)
+  HSP_NARROW_CASE(6)
   HSP_NARROW_CASE(8)
+  HSP_NARROW_CASE(12)
   HSP_NARROW_CASE(16)
 #undef HSP_NARROW_CASE
 #undef HSP_NARROW_ARGS
