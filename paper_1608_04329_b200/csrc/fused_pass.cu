@@ -637,15 +637,17 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
             float c = 0.f;
 #pragma unroll
             for (int e = 0; e < EMAX; ++e) c = fmaf(ld_shared_f32(xa + (uint32_t)(e * L) * 4u), bf[e], c);   // past p: beta = 0
-#pragma unroll 1
-            for (int off = L >> 1; off >= 1; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
+#pragma unroll
+            for (int off = 16; off >= 1; off >>= 1)
+              if (off < L) c += __shfl_xor_sync(0xffffffffu, c, off);       // L is uniform: no divergence
             s = (double)c;
           } else {
             s = 0.0;
 #pragma unroll
             for (int e = 0; e < EMAX; ++e) s = fma((double)ld_shared_x<XT>(xa + (uint32_t)(e * L) * (uint32_t)sizeof(XT)), bd[e], s);
-#pragma unroll 1
-            for (int off = L >> 1; off >= 1; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+#pragma unroll
+            for (int off = 16; off >= 1; off >>= 1)
+              if (off < L) s += __shfl_xor_sync(0xffffffffu, s, off);
           }
           if (l == 0) eta_s[st_e * RT + r] = s;
         }
