@@ -106,3 +106,18 @@ def test_host_buffer_entry_point_matches_device_entry():
     out = (torch.empty((5, wl.p), dtype=torch.float64, device="cuda"), None, torch.empty(5, dtype=torch.float64, device="cuda"))
     g.get_draws(out)
     assert np.array_equal(out[0].cpu().numpy(), b0) and np.array_equal(out[2].cpu().numpy(), t0)
+
+
+def test_non_finite_state_is_reported_not_crashed():
+    """SURVEY.md 5 (failure detection): a non-finite chain state surfaces as HSP_ENUMERIC at the next synchronising call."""
+    wl = hsp_synth.make("C2", "cuda", n_rows=3000)
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    g.sweep(2)
+    g.get_draws()
+    beta = np.zeros(wl.p); beta[3] = np.nan
+    g.set_state(beta=beta)
+    g.sweep(1)
+    with pytest.raises(hsp.HspError) as ei:
+        g.get_draws()
+    assert ei.value.code == -5
+    g.close()
