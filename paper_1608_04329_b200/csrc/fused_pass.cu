@@ -534,7 +534,7 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], kComputeWarpsAll);
       mbar_init(&eta_full[s], kComputeWarpsAll);
-      mbar_init(&z_full[s], 1);
+      mbar_init(&z_full[s], RT / 32);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -571,33 +571,34 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
       }
     }
   } else if (warp >= kComputeWarpsAll) {
-    // ===================== sampler warps: a whole tile each, lane = row =====================
+    // ===================== sampler warps: batches of 32 rows (lane = row), dealt round-robin =====================
+    // Batch gb = tile * BPT + b goes to sampler warp gb mod ns, so the BPT = RT/32 batches of a tile are sampled in
+    // parallel by different warps; z_full[stage] counts BPT arrivals.  ns <= S * BPT: a warp then never waits on a
+    // stage whose previous use has not completed its eta phase (a parity wait two phases early would pass at once).
     const int sw = warp - kComputeWarpsAll;
-    const int ns = S < kNarrowSamplers ? S : kNarrowSamplers;
+    const int BPT = RT / 32;
+    const int ns = S * BPT < kNarrowSamplers ? S * BPT : kNarrowSamplers;
+    const long long n_batches = my_tiles * BPT;
     if (sw < ns) {
-      int st = sw;
-      uint32_t ph = 0;
-      for (long long n = sw; n < my_tiles; n += ns) {
-        const long long row0 = (cta + n * grid) * RT;
-        bool waited = false;
-        for (int b = 0; b < RT; b += 32) {
-          const long long i = row0 + b + lane;
-          const bool valid = i < N;
-          const int yi = valid ? (int)y[i] : 1;
-          const double u = uniform_a(seed, (unsigned long long)(row_off + (valid ? i : 0)), sweep, TAG_Z);
-          const double ystar = 2.0 * (double)yi - 1.0;
-          if (!waited) { mbar_wait(&eta_full[st], ph); waited = true; }
-          const double eta = eta_s[st * RT + b + lane];
-          const double wpos = tnpos(ystar * eta, u);
-          const double z = valid ? ystar * wpos : 0.0;
-          z64[st * RT + b + lane] = z;
-          z32[st * RT + b + lane] = (float)z;
-          if (valid && z_out != nullptr) z_out[i] = z;
-        }
+      for (long long gb = sw; gb < n_batches; gb += ns) {
+        const long long n = gb / BPT;
+        const int b = (int)(gb - n * BPT) * 32;
+        const int st = (int)(n % S);
+        const uint32_t ph = (uint32_t)((n / S) & 1);
+        const long long i = (cta + n * grid) * RT + b + lane;
+        const bool valid = i < N;
+        const int yi = valid ? (int)y[i] : 1;
+        const double u = uniform_a(seed, (unsigned long long)(row_off + (valid ? i : 0)), sweep, TAG_Z);
+        const double ystar = 2.0 * (double)yi - 1.0;
+        mbar_wait(&eta_full[st], ph);
+        const double eta = eta_s[st * RT + b + lane];
+        const double wpos = tnpos(ystar * eta, u);
+        const double z = valid ? ystar * wpos : 0.0;
+        z64[st * RT + b + lane] = z;
+        z32[st * RT + b + lane] = (float)z;
+        if (valid && z_out != nullptr) z_out[i] = z;
         __syncwarp();
         if (lane == 0) mbar_arrive(&z_full[st]);
-        st += ns;
-        if (st >= S) { st -= S; ph ^= 1u; }
       }
     }
   } else {
