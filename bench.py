@@ -22,6 +22,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 PAPER_SWEEPS_PER_S = 10000.0 / 120.0   # 10,000 iterations in 2 min at (1e6, 1000), Titan X fp32
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused pass, from the ncu --set full captures
+# summarised in profiles/r01_g_final.md (C3: 4.001072 GB + 4.08 MB) and profiles/r01_h_narrow.md (R1: 732.2 MB read)
+NCU_TRAFFIC_BYTES = {"C3": 4005151872, "R1": 732223232}
 WORKLOAD_DESC = {
     "C1": "C1 tiny probit: N=1000, p=10, fp64 X iid N(0,1), seed 1",
     "C2": "C2 medium: N=100000, p=100, fp64 X iid N(0,1), 10 nonzeros, seed 2",
@@ -223,11 +226,7 @@ def main():
         roofline = None
         if fused_n > 0 and fused_ms > 0:
             achieved = alg_bytes / (fused_ms * 1e-3) / 1e9
-            traffic = None
-            tp = os.path.join(ROOT, "profiles", "fused_pass_traffic.json")
-            if os.path.exists(tp):
-                with open(tp) as f:
-                    traffic = json.load(f).get(args.workload)
+            traffic = NCU_TRAFFIC_BYTES.get(args.workload) if not args.paper_design else None
             roofline = {"bound": "hbm", "kernel": "paper_design(gemv+rejection+gemvT)" if args.paper_design else f"fused_pass_{variant}", "achieved": achieved, "peak": peaks["hbm_gbs"],
                         "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)", "unit": "GB/s",
                         "frac": achieved / peaks["hbm_gbs"], "frac_of_8TBps": achieved / 8000.0, "traffic": traffic,
