@@ -239,6 +239,9 @@ def main():
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": WORKLOAD_DESC[args.workload], "x_dtype": str(wl.X.dtype).replace("torch.", ""),
                            "positive_rate": wl.positive_rate, "fused_kernel": variant, "plan": plan,
+                           "arithmetic": "state, sampler, Cholesky, beta draw fp64; X fp32: eta in fp32 chains of 4 + fp64 across warps, "
+                                         "x*z in fp32 chains of 16 rows + fp64 accumulators (DESIGN.md 5)" if wl.X.dtype == torch.float32
+                                         else "fp64 throughout",
                            "l2": "X (%.1f GB) is larger than L2 and is streamed once per step" % (x_bytes / 1e9)
                            if x_bytes > 256e6 else "inputs fit L2: latency-bound config, absolute number only",
                            "launch_mode": "cuda-graph replay" if args.graph else "direct launches, 2 streams",
