@@ -121,3 +121,21 @@ def test_non_finite_state_is_reported_not_crashed():
         g.get_draws()
     assert ei.value.code == -5
     g.close()
+
+
+def test_host_entry_with_chunked_upload_matches_device_entry():
+    """hsp_create_host uploads X in row chunks on a copy stream while the Gram of the previous chunk runs (here 3
+    chunks, tensor-core Gram): the chain must be bit-identical to the device-pointer entry."""
+    wl = hsp_synth.make("C3", "cuda", n_rows=250_000, p=400)          # 400 MB of fp32 X
+    (b0, l0, t0), _ = _draws(wl, 4)
+    Xh = wl.X.cpu().pin_memory(); yh = wl.y.cpu().pin_memory()
+    g = hsp.HorseshoeProbit(Xh, yh, wl.seed, host=True)
+    g.sweep(4)
+    b, l, t = g.get_draws()
+    g.close()
+    assert np.array_equal(b, b0) and np.array_equal(l, l0) and np.array_equal(t, t0)
+    # pageable host memory takes the same path
+    g = hsp.HorseshoeProbit(wl.X.cpu(), wl.y.cpu(), wl.seed, host=True)
+    g.sweep(4)
+    assert np.array_equal(g.get_draws()[0], b0)
+    g.close()
