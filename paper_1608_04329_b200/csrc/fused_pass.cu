@@ -357,13 +357,12 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     const uint32_t zsrc0 = kF32 ? smem_u32(z32) + (uint32_t)(grp * RG * sizeof(float))
                                 : smem_u32(z64) + (uint32_t)(grp * RG * sizeof(double));
     constexpr uint32_t kEpStride = WPR * RT * sizeof(double), kZStride = RT * (kF32 ? sizeof(float) : sizeof(double));
-    uint32_t tile_e = tiles0, tile_g = tiles0;
-    uint32_t st_e = 0, st_g = 0, ph_e = 0, ph_g = 0;
     int rows_since_flush = 0;
-    const int n_my = (int)my_tiles, total_it = n_my + D;
-    for (int it = 0; it < total_it; ++it) {
-      if (it < n_my) {
-        mbar_wait_a(full0 + 8u * st_e, ph_e);
+    // eta phase on the tile in stage st (phase parity ph); x*z phase on the tile in stage st.  Called with literal
+    // stage numbers from the unrolled steady-state body below, every address below folds into an immediate.
+    auto eta_phase = [&](uint32_t st, uint32_t ph) {
+      mbar_wait_a(full0 + 8u * st, ph);
+      const uint32_t tile = tiles0 + st * sb;
         double tot;
         if constexpr (EM == 0) {
           double part[RG];
@@ -373,7 +372,7 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
           for (int c = 0; c < C; ++c) {
             Vec<XT> x[RG];
 #pragma unroll
-            for (int r = 0; r < RG; ++r) x[r].load(tile_e + r * rb + coff[c]);
+            for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
 #pragma unroll
             for (int r = 0; r < RG; ++r) part[r] += x[r].dot(breg[c]);
           }
@@ -386,22 +385,21 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
           for (int c = 0; c < C; ++c) {
             Vec<XT> x[RG];
 #pragma unroll
-            for (int r = 0; r < RG; ++r) x[r].load(tile_e + r * rb + coff[c]);
+            for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
 #pragma unroll
             for (int r = 0; r < RG; ++r) part[r] += x[r].dotf(bregf[c]);
           }
           tot = (double)warp_reduce_rows<float, RG>(part, lane);
         }
-        if (writer) st_shared_f64(epart0 + st_e * kEpStride, tot);
-        __syncwarp();
-        if (lane == 0) mbar_arrive_a(etaf0 + 8u * st_e);
-        tile_e += sb;
-        if (++st_e == (uint32_t)S) { st_e = 0; ph_e ^= 1u; tile_e = tiles0; }
-      }
-      if (it >= D) {
-        mbar_wait_a(zf0 + 8u * st_g, ph_g);
+      if (writer) st_shared_f64(epart0 + st * kEpStride, tot);
+      __syncwarp();
+      if (lane == 0) mbar_arrive_a(etaf0 + 8u * st);
+    };
+    auto xz_phase = [&](uint32_t st, uint32_t ph) {
+      mbar_wait_a(zf0 + 8u * st, ph);
+      const uint32_t tile = tiles0 + st * sb;
         Acc zr[RG];
-        const uint32_t zp = zsrc0 + st_g * kZStride;
+        const uint32_t zp = zsrc0 + st * kZStride;
         if constexpr (kF32) {
           if constexpr (RG % 4 == 0) {
 #pragma unroll
@@ -430,26 +428,54 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         for (int c = 0; c < C; ++c) {
           Vec<XT> x[RG];
 #pragma unroll
-          for (int r = 0; r < RG; ++r) x[r].load(tile_g + r * rb + coff[c]);
+          for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
 #pragma unroll
           for (int r = 0; r < RG; ++r) x[r].axpy(zr[r], acc[c]);
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive_a(empty0 + 8u * st_g);
-        tile_g += sb;
-        if (++st_g == (uint32_t)S) { st_g = 0; ph_g ^= 1u; tile_g = tiles0; }
-        if constexpr (kF32) {
-          rows_since_flush += RG;
-          if (rows_since_flush >= kFlushRows) {
-            rows_since_flush = 0;
+      __syncwarp();
+      if (lane == 0) mbar_arrive_a(empty0 + 8u * st);
+      if constexpr (kF32) {
+        rows_since_flush += RG;
+        if (rows_since_flush >= kFlushRows) {
+          rows_since_flush = 0;
 #pragma unroll
-            for (int c = 0; c < C; ++c)
+          for (int c = 0; c < C; ++c)
 #pragma unroll
-              for (int v = 0; v < V; ++v) { acc64[c][v] += (double)acc[c][v]; acc[c][v] = (Acc)0; }
-          }
+            for (int v = 0; v < V; ++v) { acc64[c][v] += (double)acc[c][v]; acc[c][v] = (Acc)0; }
         }
       }
+    };
+    uint32_t st_e = 0, st_g = 0, ph_e = 0, ph_g = 0;
+    const int n_my = (int)my_tiles, total_it = n_my + D;
+    int it = 0;
+    auto generic_iter = [&]() {
+      if (it < n_my) {
+        eta_phase(st_e, ph_e);
+        if (++st_e == (uint32_t)S) { st_e = 0; ph_e ^= 1u; }
+      }
+      if (it >= D) {
+        xz_phase(st_g, ph_g);
+        if (++st_g == (uint32_t)S) { st_g = 0; ph_g ^= 1u; }
+      }
+      ++it;
+    };
+    constexpr bool kUnrollRing = (C == 1);   // wider per-thread state spills when the body is unrolled 7 times
+    if (kUnrollRing && S == 7 && D == 3 && n_my >= 14) {
+      // steady state unrolled over the ring (the shape of C3, C4, C5: 7 stages of 32 KB, lag 3): iteration 7k + s runs
+      // the eta phase on stage s and the x*z phase on stage (s + 4) mod 7 -- no wrap logic, no loop conditions.
+      for (int q = 0; q < 7; ++q) generic_iter();                 // it = 7: st_e = 0, st_g = 4
+      uint32_t phb = ph_e;                                        // parity of k = it / 7
+      for (; it + 7 <= n_my; it += 7) {
+#pragma unroll
+        for (int u = 0; u < 7; ++u) {
+          eta_phase((uint32_t)u, phb);
+          xz_phase((uint32_t)((u + 4) % 7), u >= 3 ? phb : phb ^ 1u);
+        }
+        phb ^= 1u;
+      }
+      ph_e = phb; ph_g = phb ^ 1u; st_e = 0; st_g = 4;            // state of the generic loop at it = 7k
     }
+    while (it < total_it) generic_iter();
     (void)tiles_end;
 #pragma unroll
     for (int c = 0; c < C; ++c) {
@@ -812,7 +838,7 @@ static bool tma_shape(int vec, int prefer_w, TmaShape* out) {
   const TmaShape shapes[] = {{8, 1, 256}, {4, 2, 256}, {4, 1, 512}, {2, 2, 512}, {1, 4, 512}, {1, 8, 512}};
   for (const TmaShape& sh : shapes) {
     if (vec > sh.C * sh.W) continue;
-    if (prefer_w && sh.W != prefer_w && vec <= 512 && vec > 256) continue;   // p in (256 V, 512 V]: two candidates
+    if (sh.W != (prefer_w ? prefer_w : 512) && vec <= 512 && vec > 256) continue;   // p in (256 V, 512 V]: two candidates, 16 warps across the row by default
     *out = sh;
     return true;
   }
