@@ -63,8 +63,12 @@ enum {
  *   y       DEVICE N bytes, each 0 or 1.  BORROWED likewise.  Any other value -> HSP_EINVAL.
  *   N >= 2, p >= 1, seed any 64-bit value.
  *   stream  cudaStream_t passed as void* (NULL = the legacy default stream).
- * Runs the Gram kernel (G = X^T X, fp64, exact products) on the stream and returns after it is
- * enqueued and validated.  Errors: HSP_EINVAL (arguments), HSP_ENOMEM, HSP_ECUDA.               */
+ * Computes G = X^T X (fp64 result) on the stream and returns after it has completed: fp64 X and small problems by
+ * exact fp64 products; fp32 X with N p^2 >= 2e10 on the tcgen05 tensor cores (split-bf16 products, fp64 flush:
+ * |dG| <= 1e-6 max|G|; option "gram_tc" forces either).  The launch plan (kernel variant, tile shape, SMs of the
+ * Cholesky branch) is fixed here from (N, p, dtype) and the plan-time options in force (hsp_set_option).
+ * One process may hold chains on several devices: the chain lives on the device current at create.
+ * Errors: HSP_EINVAL (arguments), HSP_ENOMEM, HSP_ECUDA.                                        */
 int hsp_create(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N, int p,
                unsigned long long seed, void* stream);
 
@@ -105,6 +109,22 @@ int hsp_sweep(hsp_state* s, long long n_iter);
  * Synchronises the stream.                                                                       */
 int hsp_get_draws(const hsp_state* s, double* beta, double* lambda, double* tau);
 
+/* Asynchronous download of the Monte Carlo output ("Monte Carlo output is downloaded off of the GPU
+ * at the same time as updates for other variables are computed").  Registers a HOST ring of `capacity` sweeps:
+ * host_beta[capacity*p], host_lambda[capacity*p], host_tau[capacity] (any may be NULL; BORROWED until the next
+ * hsp_set_output / hsp_destroy; pinned memory -- cudaHostAlloc / cudaHostRegister -- keeps the copies asynchronous).
+ * From then on every sweep enqueued by hsp_sweep / hsp_sweep_end is also copied to ring row (r mod capacity), r = 0,
+ * 1, ... counting sweeps since this call, by a copy stream that waits on an event recorded after the sweep's beta
+ * draw -- in blocks of a few sweeps (>= 64 KB), with no host synchronisation and without delaying the next sweep.
+ * capacity = 0 or all pointers NULL switches the download off.  hsp_get_draws is unaffected.
+ *   hsp_output_ready  non-blocking: *rows = number of sweeps (since hsp_set_output) that have landed on the host.
+ *   hsp_output_wait   blocks until every sweep enqueued so far has landed; *rows (may be NULL) = their number;
+ *                     returns the device status like hsp_sync (HSP_ENOTPD / HSP_ENUMERIC).
+ * Errors: HSP_EINVAL, HSP_ECUDA.                                                                  */
+int hsp_set_output(hsp_state* s, double* host_beta, double* host_lambda, double* host_tau, long long capacity);
+int hsp_output_ready(hsp_state* s, long long* rows);
+int hsp_output_wait(hsp_state* s, long long* rows);
+
 /* Synchronise the stream and report device-side status (HSP_OK, HSP_ENOTPD, HSP_ENUMERIC).       */
 int hsp_sync(const hsp_state* s);
 
@@ -140,8 +160,25 @@ long long hsp_get_launch_count(const hsp_state* s);
  * whether the two run side by side on disjoint SMs (1) or one after the other (0), and the cost-model
  * estimate of the Cholesky branch in microseconds.  HOST pointers, any may be NULL.               */
 int hsp_get_plan(const hsp_state* s, int* fused_ctas, int* chol_ctas, int* overlap, double* chol_est_us);
-/* Name of the fused-pass kernel variant selected for this (dtype, p): "tma" or "generic".        */
+/* Name of the fused-pass kernel variant selected for this (dtype, N, p): "tma" (rows of >= 128 16-byte vectors),
+ * "tma-narrow" (narrower rows, p <= 511, X >= 2 MB) or "generic" (everything else).                */
 const char* hsp_fused_variant(const hsp_state* s);
+
+/* Plan-time and launch-mode options (tests and tuning; the defaults are what bench.py measures).  The library reads
+ * NO environment variables.  state == NULL sets the process-wide default that chains created AFTERWARDS copy at
+ * create (thread-safe); value < 0 restores the automatic choice; key == NULL (state == NULL) restores all.  With a
+ * state only "no_pdl" may change (the launch plan of an existing chain is fixed).  Keys:
+ *   fused_eta 0|2      eta arithmetic for fp32 X: exact fp64 | fp32 chains of 4 (default)
+ *   fused_grid, fused_stages, fused_lag, fused_w (256|512), narrow_rt      grid, ring depth, lag, threads across a
+ *                      row, rows per narrow tile of the fused pass
+ *   fused_variant 0|1  force the generic kernel | allow the wide TMA kernel below 128 vectors per row
+ *   fused_narrow 0     disable the narrow kernel
+ *   chol_ctas K, chol_sb (tiles per inverse super-block), chol_trace 1     Cholesky branch
+ *   gram_tc 0|1        exact | tensor-core Gram
+ *   no_pdl 1           tail kernels without programmatic dependent launch
+ * Errors: HSP_EINVAL (unknown key, plan-time key with a state).                                     */
+int hsp_set_option(hsp_state* s, const char* key, long long value);
+int hsp_get_option(const hsp_state* s, const char* key, long long* value);
 
 /* Device unit-test hooks (one thread per element; DEVICE pointers):
  *   philox : out[4n] = Philox-4x32-10(ctr[4n], key[2n])
@@ -157,7 +194,7 @@ int hsp_dbg_cheng(double alpha, unsigned long long seed, unsigned sweep0, double
 
 
 /* Measurement hook for rows c, d1: the static schedule of the Cholesky task graph and, if
- * the environment variable HSP_CHOL_TRACE=1 was set when the chain was created, the device timestamps of
+ * option "chol_trace" = 1 was in force when the chain was created, the device timestamps of
  * the tasks of the last sweep.  rows: HOST, capacity x 12 long long per task, in schedule order:
  * {type, i, j, kbeg, kend, slot_in, slot_out, cta, t_start_ns, t_kloop_end_ns, t_end_ns, 0} (timestamps 0
  * without the trace).  Returns the number of tasks (rows may be NULL to query it), or a negative status.

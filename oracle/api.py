@@ -6,7 +6,7 @@ import numpy as np
 from . import build as _build
 
 F32, F64 = 0, 1
-STORE_Z, FREEZE_SCALES, FREEZE_Z, LITERAL_Z, FREEZE_BETA = 1, 2, 4, 8, 16
+STORE_Z, FREEZE_SCALES, FREEZE_Z, LITERAL_Z, FREEZE_BETA, ROW_CHUNKS = 1, 2, 4, 8, 16, 32
 TAG_Z, TAG_LAMBDA, TAG_TAU, TAG_E, TAG_NU, TAG_XI = 0, 1, 2, 3, 4, 5
 
 _lib = None
@@ -63,8 +63,14 @@ def lib():
         L.hspo_get_timing.argtypes = [C.c_void_p, dp, dp]
         L.hspo_get_literal_trials.argtypes = [C.c_void_p]
         L.hspo_get_literal_trials.restype = C.c_longlong
+        L.hspo_max_threads.restype = C.c_int
         _lib = L
     return _lib
+
+
+def max_threads():
+    """Threads the timing-only ROW_CHUNKS mode uses."""
+    return lib().hspo_max_threads()
 
 
 def _ptr(a):

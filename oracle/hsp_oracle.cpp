@@ -22,6 +22,13 @@
 // All arithmetic is fp64; the special-function inversions run in long double.  Loops are the
 // textbook ones (i ascending, j ascending); nothing is blocked, fused or reordered.
 //
+// TIMING-ONLY mode FLAG_ROW_CHUNKS (never used by a parity test as the reference): steps 1-3 run over FIXED
+// chunks of 4096 rows, the chunks dealt to the host cores by OpenMP, each chunk keeping its own partial of
+// X^T z, and the partials are added in chunk order -- the same row arithmetic, the analogue of the paper's
+// 16-thread workstation code (SURVEY.md 8(d) "oracle timing (ii)").  The result does not
+// depend on the number of threads; it differs from the default path by the summation order of g only
+// (pinned by tests/test_oracle_chain.py::test_row_chunk_mode_matches_default).
+//
 // Random numbers: the paper says only "use Philox".  The contract (DESIGN.md
 // "Random-number contract") is Philox-4x32-10 with counter (idx_lo, idx_hi, sweep, tag) and key
 // (seed_lo, seed_hi); one Philox call per variate.  This file has its own implementation.
@@ -45,8 +52,12 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <new>
 #include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 namespace {
 
@@ -241,7 +252,8 @@ void solve_lower_t(const double* L, int p, double* b) {     // L^T x = b, back s
 
 enum { F32 = 0, F64 = 1 };
 enum { FLAG_STORE_Z = 1u, FLAG_FREEZE_SCALES = 2u, FLAG_FREEZE_Z = 4u, FLAG_LITERAL_Z = 8u,
-       FLAG_FREEZE_BETA = 16u };
+       FLAG_FREEZE_BETA = 16u, FLAG_ROW_CHUNKS = 32u };
+constexpr int64_t kRowChunk = 4096;
 
 struct Chain {
   const void* X; int dtype; const uint8_t* y; int64_t N; int p; uint64_t seed;
@@ -267,7 +279,30 @@ int sweep_once(Chain& c) {
   const int p = c.p; const int64_t N = c.N;
   const uint32_t k = (uint32_t)(++c.sweep);
   const double t0 = now_s();
-  if (!(c.flags & FLAG_FREEZE_Z)) {
+  if (!(c.flags & FLAG_FREEZE_Z) && (c.flags & FLAG_ROW_CHUNKS) && !(c.flags & FLAG_LITERAL_Z)) {
+    // timing-only: steps 1-3 over fixed row chunks on all cores (see the header); same row arithmetic as below
+    const int64_t n_chunks = (N + kRowChunk - 1) / kRowChunk;
+    std::vector<double> part((size_t)n_chunks * p, 0.0);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t ch = 0; ch < n_chunks; ++ch) {
+      const int64_t i0 = ch * kRowChunk, i1 = std::min(N, i0 + kRowChunk);
+      double* gp = part.data() + (size_t)ch * p;
+      for (int64_t i = i0; i < i1; ++i) {
+        double s = 0.0;
+        for (int j = 0; j < p; ++j) s += c.x(i, j) * c.beta[j];
+        c.eta[i] = s;
+        const double ystar = 2.0 * (double)c.y[i] - 1.0;
+        double u;
+        uniforms(c.seed, (uint64_t)i, k, TAG_Z, &u, nullptr);
+        const double zi = ystar * tnpos(ystar * s, u);
+        c.z[i] = zi;
+        for (int j = 0; j < p; ++j) gp[j] += c.x(i, j) * zi;
+      }
+    }
+    for (int j = 0; j < p; ++j) c.g[j] = 0.0;
+    for (int64_t ch = 0; ch < n_chunks; ++ch)
+      for (int j = 0; j < p; ++j) c.g[j] += part[(size_t)ch * p + j];
+  } else if (!(c.flags & FLAG_FREEZE_Z)) {
     // 1. eta = X beta
     for (int64_t i = 0; i < N; ++i) {
       double s = 0.0;
@@ -482,5 +517,13 @@ int hspo_get_timing(const void* s, double* t_rows, double* t_rest) {
   return 0;
 }
 long long hspo_get_literal_trials(const void* s) { return ((const Chain*)s)->literal_trials; }
+// threads the FLAG_ROW_CHUNKS mode uses (1 when built without OpenMP)
+int hspo_max_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
 
 }  // extern "C"

@@ -77,6 +77,11 @@ def lib():
     L.hsp_dbg_cheng.argtypes = [C.c_double, ull, C.c_uint, vp, ll, vp]
     L.hsp_dbg_chol_trace.argtypes = [vp, vp, ll]
     L.hsp_get_plan.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), dp]
+    L.hsp_set_option.argtypes = [vp, C.c_char_p, ll]
+    L.hsp_get_option.argtypes = [vp, C.c_char_p, C.POINTER(ll)]
+    L.hsp_set_output.argtypes = [vp, vp, vp, vp, ll]
+    L.hsp_output_ready.argtypes = [vp, C.POINTER(ll)]
+    L.hsp_output_wait.argtypes = [vp, C.POINTER(ll)]
     L.hsp_dbg_chol_trace.restype = ll
     _lib = L
     return L
@@ -89,6 +94,21 @@ def _check(rc):
 
 def _np(a):
     return a.ctypes.data_as(C.c_void_p)
+
+
+def set_option(key, value):
+    """hsp_set_option(NULL, key, value): process-wide default for chains created afterwards (value < 0: automatic)."""
+    _check(lib().hsp_set_option(None, key.encode(), int(value)))
+
+
+def reset_options():
+    _check(lib().hsp_set_option(None, None, 0))
+
+
+def get_option(key):
+    v = C.c_longlong()
+    _check(lib().hsp_get_option(None, key.encode(), C.byref(v)))
+    return v.value
 
 
 def _stream_handle(stream):
@@ -145,6 +165,30 @@ class HorseshoeProbit:
 
     def sync(self):
         _check(lib().hsp_sync(self._h))
+
+    def stream_handle(self):
+        """The cudaStream_t (as int) this chain enqueues on."""
+        return int(self._stream.cuda_stream)
+
+    def set_option(self, key, value):
+        _check(lib().hsp_set_option(self._h, key.encode(), int(value)))
+
+    # ---- asynchronous download of the draws into a pinned host ring (hsp_set_output)
+    def set_output(self, beta, lam, tau, capacity):
+        """beta [capacity, p], lam [capacity, p], tau [capacity]: pinned host tensors / arrays (any may be None)."""
+        self._out = (beta, lam, tau)                   # borrowed by the library: keep alive
+        ptrs = [None if t is None else (t.data_ptr() if hasattr(t, "data_ptr") else _np(t)) for t in self._out]
+        _check(lib().hsp_set_output(self._h, *ptrs, int(capacity)))
+
+    def output_ready(self):
+        n = C.c_longlong()
+        _check(lib().hsp_output_ready(self._h, C.byref(n)))
+        return n.value
+
+    def output_wait(self):
+        n = C.c_longlong()
+        _check(lib().hsp_output_wait(self._h, C.byref(n)))
+        return n.value
 
     # ---- row-sharded chains: hsp_sweep_prepare / _begin / _end and the two buffers the caller all-reduces
     def sweep_prepare(self, n_iter):
@@ -233,7 +277,7 @@ class HorseshoeProbit:
         return {"fused_ctas": a.value, "chol_ctas": b.value, "overlap": bool(c.value), "chol_est_us": d.value}
 
     def chol_trace(self):
-        """Static tile schedule of rows c, d1 (and timestamps, with HSP_CHOL_TRACE=1): int64 [n_tasks, 12]."""
+        """Static tile schedule of rows c, d1 (and timestamps, with option chol_trace = 1): int64 [n_tasks, 12]."""
         n = lib().hsp_dbg_chol_trace(self._h, None, 0)
         if n < 0:
             _check(int(n))

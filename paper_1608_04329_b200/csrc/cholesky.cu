@@ -643,25 +643,20 @@ beta_keep_kernel(const double* __restrict__ beta, int p, Ctl* __restrict__ ctl) 
   if (threadIdx.x == 0) ctl->sweep = k;
 }
 
-static int env_int2(const char* name, int dflt) {
-  const char* v = getenv(name);
-  return (v && *v) ? atoi(v) : dflt;
-}
-
 // Build the static schedule and decide how many SMs the Cholesky branch gets.  When the cost model says the
 // branch hides behind the fused pass on K SMs of its own (the pass keeps num_sms - K), the smallest such K
 // is taken; otherwise the branch uses every SM and runs before/after the pass.
-cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_estimate) {
+cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_estimate, const Options& opt) {
   pl->p = p; pl->nt = chol_tiles(p); pl->P = chol_ld(p);
   const int nt = pl->nt;
   // Inverse factor: the whole W = L^-1 for nt <= 20 (d2 is then two matrix-vector products); for larger p only the
   // diagonal super-blocks of sb x sb tiles (the full inverse would double the flops) and d2 is a block substitution.
-  const int sb_env = env_int2("HSP_CHOL_SB", 0);
+  const int sb_env = opt_or(opt.chol_sb, 0);
   const int sb = sb_env > 0 ? std::min(sb_env, nt) : (nt <= 20 ? nt : 8);
   pl->sb = sb;
   const long long tile_tasks = (long long)nt * nt;
   CholSchedule best;
-  int k_env = env_int2("HSP_CHOL_CTAS", 0);
+  int k_env = opt_or(opt.chol_ctas, 0);
   if (k_env > num_sms) k_env = num_sms;
   if (k_env > 0) {
     best = chol_build_schedule(nt, sb, (int)std::min<long long>(k_env, tile_tasks));
@@ -705,7 +700,7 @@ cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_e
   if (e == cudaSuccess) e = cudaMalloc(&pl->d_ws, (size_t)std::max(1, best.n_slots) * CT * CT * sizeof(double));
   if (e == cudaSuccess) e = cudaMemcpy(pl->d_tasks, best.tasks.data(), best.tasks.size() * sizeof(CholTask), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(pl->d_list_off, best.list_off.data(), best.list_off.size() * sizeof(int), cudaMemcpyHostToDevice);
-  if (e == cudaSuccess && env_int2("HSP_CHOL_TRACE", 0)) {
+  if (e == cudaSuccess && opt_or(opt.chol_trace, 0)) {
     e = cudaMalloc(&pl->d_trace, best.tasks.size() * 4 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(pl->d_trace, 0, best.tasks.size() * 4 * sizeof(unsigned long long));
   }
@@ -749,10 +744,9 @@ static cudaError_t launch_pdl(void (*kern)(KArgs...), int grid, int block, cudaS
 }
 
 cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g, double* tv, double* beta, int p,
-                              unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches) {
+                              unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches, bool pdl) {
   const int P = chol_ld(p);
   const int grid = (p + kGemvWarps - 1) / kGemvWarps;
-  static const bool pdl = env_int2("HSP_NO_PDL", 0) == 0;
   cudaError_t e = launch_pdl(beta_gemv1_kernel, grid, kGemvWarps * 32, st, pdl, W, g, tv, p, P, seed, (const Ctl*)ctl);
   if (e != cudaSuccess) return e;
   e = launch_pdl(beta_gemv2_kernel, grid, kGemvWarps * 32, st, pdl, Wt, (const double*)tv, beta, p, P, ctl);
@@ -762,9 +756,8 @@ cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g
 
 cudaError_t beta_block_solve_launch(const double* L, const double* Lt, const double* W, const double* Wt, const double* g,
                                     double* tv, double* rv, double* beta, int p, int sb, unsigned long long seed, Ctl* ctl,
-                                    cudaStream_t st, long long* launches) {
+                                    cudaStream_t st, long long* launches, bool pdl) {
   const int P = chol_ld(p), B = sb * CT, nsb = (P + B - 1) / B;
-  static const bool pdl = env_int2("HSP_NO_PDL", 0) == 0;
   const Ctl* cc = ctl;
   cudaError_t e = cudaSuccess;
   auto launch = [&](const double* M, int row0, int nrows, int c0, int c1, int tri, const double* x, const double* in,

@@ -181,11 +181,6 @@ __device__ __forceinline__ int row_of_lane(int lane) {
   return row;
 }
 
-static int env_int(const char* name, int dflt) {
-  const char* v = getenv(name);
-  return (v && *v) ? atoi(v) : dflt;
-}
-
 constexpr int kComputeWarpsAll = 16;             // compute warps per CTA
 constexpr int kComputeThreadsAll = kComputeWarpsAll * 32;
 constexpr int kSamplerWarps = 4;
@@ -845,7 +840,7 @@ static bool tma_shape(int vec, int prefer_w, TmaShape* out) {
   return false;
 }
 
-static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* X, FusedPlan* pl) {
+static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* X, const Options& opt, FusedPlan* pl) {
   const size_t elem = dtype == kF32 ? 4 : 8;
   const size_t row_bytes = (size_t)p * elem;
   // tiny problems (C1) are launch-bound: the generic kernel has no 224 KB ring to set up
@@ -856,26 +851,26 @@ static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* 
   if (E > 16) return false;
   int RT = (int)(56000 / row_bytes) / 32 * 32;      // ~50 KB stages (4 fit): the per-tile overhead is what limits narrow rows
   RT = RT < 32 ? 32 : RT > 256 ? 256 : RT;
-  if (env_int("HSP_NARROW_RT", 0) > 0) RT = env_int("HSP_NARROW_RT", 0) / 32 * 32;
+  if (opt.narrow_rt > 0) RT = opt.narrow_rt / 32 * 32;
   const size_t stage_bytes = narrow_stage_bytes(RT, row_bytes);
   const size_t budget = 227 * 1024;
-  int S = env_int("HSP_FUSED_STAGES", 0);
+  int S = opt_or(opt.fused_stages, 0);
   if (S <= 0) {
     S = 8;
     while (S > 2 && NarrowSmemLayout(S, RT, p, stage_bytes).total > budget) --S;
   }
   if (S < 3 || NarrowSmemLayout(S, RT, p, stage_bytes).total > budget) return false;
-  int D = env_int("HSP_FUSED_LAG", 0);
+  int D = opt_or(opt.fused_lag, 0);
   if (D <= 0) D = (S - 1) / 2 > 2 ? (S - 1) / 2 : 2;
   if (D > S - 2) D = S - 2;
   if (D < 1) D = 1;
   pl->variant = 2;
   pl->rows_per_tile = RT; pl->chunks = E <= 4 ? 4 : E <= 6 ? 6 : E <= 8 ? 8 : E <= 12 ? 12 : 16; pl->width = L; pl->stages = S; pl->lag = D;
   pl->groups = 1;
-  int em = dtype == kF32 ? env_int("HSP_FUSED_ETA", 2) : 0;
+  int em = dtype == kF32 ? opt_or(opt.fused_eta, 2) : 0;
   pl->eta_mode = (em == 0) ? 0 : 2;
   pl->n_tiles = (N + RT - 1) / RT;
-  int grid = env_int("HSP_FUSED_GRID", num_sms);
+  int grid = opt.fused_grid > 0 ? opt.fused_grid : num_sms;
   if ((long long)grid > pl->n_tiles) grid = (int)pl->n_tiles;
   pl->grid = grid; pl->block = kNarrowThreads;
   pl->smem = NarrowSmemLayout(S, RT, p, stage_bytes).total;
@@ -887,13 +882,9 @@ static cudaError_t launch_narrow(const FusedPlan& pl, const void* X, const unsig
                                  unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                                  double* z_out, cudaStream_t st) {
   auto kern = fused_pass_narrow<XT, EMAX, EM>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  if (N < 0) return cudaSuccess;
+  // prepare-only call (hsp_create, once per chain, outside stream capture): the attribute is per DEVICE, so it is
+  // set for the current device every time a chain is created, not once per process
+  if (N < 0) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
   kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
                                           pl.stages, pl.lag, pl.rows_per_tile, pl.width, pl.n_tiles, pl.row_offset);
   return cudaGetLastError();
@@ -921,43 +912,43 @@ static cudaError_t dispatch_narrow(const FusedPlan& pl, const void* X, const uns
   return cudaErrorInvalidValue;
 }
 
-FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X) {
+FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X, const Options& opt) {
   FusedPlan pl{};
   const size_t elem = dtype == kF32 ? 4 : 8;
   const size_t row_bytes = (size_t)p * elem;
   const bool aligned = (row_bytes % 16 == 0) && ((reinterpret_cast<uintptr_t>(X) & 15) == 0);
   const int vec = (int)(row_bytes / 16);
   const bool wide = vec >= 128;
-  const int force = env_int("HSP_FUSED_VARIANT", -1);
+  const int force = opt.fused_variant;
   TmaShape sh{};
-  if (aligned && (wide || force == 1) && force != 0 && tma_shape(vec, env_int("HSP_FUSED_W", 0), &sh)) {
+  if (aligned && (wide || force == 1) && force != 0 && tma_shape(vec, opt_or(opt.fused_w, 0), &sh)) {
     const int RT = sh.RT, WPR = sh.W / 32;
     const size_t stage_bytes = ((size_t)RT * row_bytes + 127) & ~(size_t)127;
     const size_t budget = 227 * 1024;
-    int S = env_int("HSP_FUSED_STAGES", 0);
+    int S = opt_or(opt.fused_stages, 0);
     if (S <= 0) {
       S = 12;
       while (S > 2 && TmaSmemLayout(S, RT, WPR, stage_bytes).total > budget) --S;
     }
     if (S >= 3 && TmaSmemLayout(S, RT, WPR, stage_bytes).total <= budget) {
-      int D = env_int("HSP_FUSED_LAG", 0);
+      int D = opt_or(opt.fused_lag, 0);
       if (D <= 0) D = (S - 1) / 2;
       if (D > S - 2) D = S - 2;
       if (D < 1) D = 1;
       pl.variant = 1;
       pl.rows_per_tile = RT; pl.chunks = sh.C; pl.width = sh.W; pl.stages = S; pl.lag = D;
       pl.groups = kComputeThreadsAll / sh.W;
-      int em = dtype == kF32 ? env_int("HSP_FUSED_ETA", 2) : 0;
+      int em = dtype == kF32 ? opt_or(opt.fused_eta, 2) : 0;
       pl.eta_mode = (em == 0) ? 0 : 2;
       pl.n_tiles = (N + RT - 1) / RT;
-      int grid = env_int("HSP_FUSED_GRID", num_sms);
+      int grid = opt.fused_grid > 0 ? opt.fused_grid : num_sms;
       if ((long long)grid > pl.n_tiles) grid = (int)pl.n_tiles;
       pl.grid = grid; pl.block = kTmaThreads;
       pl.smem = TmaSmemLayout(S, RT, WPR, stage_bytes).total;
       return pl;
     }
   }
-  if (force != 0 && env_int("HSP_FUSED_NARROW", 1) && narrow_plan(dtype, N, p, num_sms, X, &pl)) return pl;
+  if (force != 0 && opt_or(opt.fused_narrow, 1) && narrow_plan(dtype, N, p, num_sms, X, opt, &pl)) return pl;
   pl = FusedPlan{};
   pl.variant = 0;
   pl.n_tiles = (N + kGenThreads - 1) / kGenThreads;
@@ -973,13 +964,8 @@ static cudaError_t launch_tma(const FusedPlan& pl, const void* X, const unsigned
                               unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                               double* z_out, cudaStream_t st) {
   auto kern = fused_pass_tma<XT, RT, C, W, EM>;
-  static bool configured = false;   // per instantiation
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  if (N < 0) return cudaSuccess;     // prepare-only call (sets the attribute outside stream capture)
+  // prepare-only call (hsp_create, once per chain, outside stream capture): per-device attribute, see launch_narrow
+  if (N < 0) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
   kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
                                           pl.stages, pl.lag, pl.n_tiles, pl.row_offset);
   return cudaGetLastError();

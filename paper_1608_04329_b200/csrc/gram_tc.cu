@@ -254,11 +254,9 @@ gram_tc_kernel(const float* __restrict__ X, long long N, int p, double* __restri
 int gram_tc_tiles(int p) { const int ts = (p + kTcTile - 1) / kTcTile; return ts * (ts + 1) / 2; }
 
 cudaError_t gram_tc_chunk_launch(const GramPlan& g, int chunk, const float* X, long long N, int p, double* scratch, cudaStream_t st) {
-  static bool configured = false;
-  if (!configured) {
+  if (chunk == 0) {   // per-device attribute: set for the current device at every create (chunk 0), not once per process
     cudaError_t e = cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmem);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   dim3 grid(gram_tc_tiles(p), g.slots_per_chunk);
   gram_tc_kernel<<<grid, kTcThreads, kTcSmem, st>>>(X, N, p, scratch, chunk * g.slots_per_chunk, g.rows_per_slot);

@@ -13,6 +13,7 @@
 #include <vector>
 #include <algorithm>
 #include <new>
+#include <mutex>
 #include "../../include/hsp.h"
 #include "hsp_device.cuh"
 #include "hsp_internal.h"
@@ -20,7 +21,9 @@
 using namespace hsp;
 
 static thread_local std::string g_err;
-static thread_local long long g_pending_row_offset = 0;   // hsp_create_shard -> hsp_create
+// process-wide defaults of the plan-time options (hsp_set_option with state == NULL); a chain copies them at create
+static std::mutex g_opt_mutex;
+static Options g_default_options;
 static int fail(int code, const std::string& msg) { g_err = msg; return code; }
 static int cuda_fail(cudaError_t e, const char* what) {
   g_err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -58,6 +61,18 @@ struct hsp_state {
   long long launches = 0;
   std::vector<cudaEvent_t> tev;   // event pairs around the fused pass (direct-launch mode)
   size_t tev_used = 0; double fused_ms_sum = 0.0; long long fused_n = 0;
+  Options opt{};                  // plan-time options, copied from the process defaults at create
+  // asynchronous download of the draws (hsp_set_output): host ring + copy stream
+  double *o_beta = nullptr, *o_lambda = nullptr, *o_tau = nullptr;   // HOST, borrowed
+  long long o_cap = 0, o_rows = 0;         // ring capacity in sweeps; rows enqueued since hsp_set_output
+  long long o_block = 1;                   // sweeps per download block
+  long long o_pending_first = 0, o_pending = 0;   // history rows of the current call not yet handed to the copy stream
+  cudaStream_t stream3 = nullptr;          // copy stream
+  std::vector<cudaEvent_t> o_ev_sweep;     // recorded on the compute stream after the last sweep of a block
+  std::vector<cudaEvent_t> o_ev_done;      // recorded on the copy stream after the block has landed on the host
+  std::vector<long long> o_ev_rows;        // o_rows once that block is complete
+  size_t o_ev_next = 0, o_ev_checked = 0; long long o_completed = 0;   // blocks enqueued / known landed; rows landed
+  cudaEvent_t o_last_done = nullptr;       // the most recent o_ev_done (not owned)
 };
 
 static int prepare_history(hsp_state* s, long long n_iter);
@@ -68,6 +83,9 @@ static void free_state(hsp_state* s) {
   for (cudaEvent_t e : s->tev) cudaEventDestroy(e);
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
   if (s->ev_join) cudaEventDestroy(s->ev_join);
+  for (cudaEvent_t e : s->o_ev_sweep) cudaEventDestroy(e);
+  for (cudaEvent_t e : s->o_ev_done) cudaEventDestroy(e);
+  if (s->stream3) cudaStreamDestroy(s->stream3);
   if (s->stream2) cudaStreamDestroy(s->stream2);
   if (s->own_stream) cudaStreamDestroy(s->own_stream);
   void* ptrs[] = {s->own_X, s->own_y, s->G, s->L, s->Lt, s->rv, s->W, s->Wt, s->beta, s->lam_inv2, s->nu_inv, s->g, s->tv, s->partial,
@@ -94,7 +112,9 @@ static int drain_fused_events(hsp_state* s) {
 // phases: 1 = up to and including the reduction of X^T z (and the whole side branch), 2 = the beta draw, 3 = both.
 static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels, int phases = 3) {
   cudaStream_t A = s->stream;
-  const bool serial = (s->flags & HSP_SERIAL) != 0;
+  // one stream when asked for, and when the plan found no way to hide the Cholesky branch (c, d1) behind the pass
+  // (p = 4000: both kernels want every SM; launched on two streams their CTAs would interleave at random)
+  const bool serial = (s->flags & HSP_SERIAL) != 0 || !s->chol.overlap;
   cudaStream_t B = serial ? A : s->stream2;
   const bool do_z = !(s->flags & HSP_FREEZE_Z), do_scales = !(s->flags & HSP_FREEZE_SCALES),
              do_beta = !(s->flags & HSP_FREEZE_BETA);
@@ -143,8 +163,9 @@ static int enqueue_sweep(hsp_state* s, bool timed, long long* kernels, int phase
   if (phases == 1) return HSP_OK;
 draw:
   if (do_beta && s->chol.sb < s->chol.nt)
-    CK(beta_block_solve_launch(s->L, s->Lt, s->W, s->Wt, s->g, s->tv, s->rv, s->beta, s->p, s->chol.sb, s->seed, s->ctl, A, kernels));
-  else if (do_beta) CK(beta_solve_launch(s->W, s->Wt, s->g, s->tv, s->beta, s->p, s->seed, s->ctl, A, kernels));
+    CK(beta_block_solve_launch(s->L, s->Lt, s->W, s->Wt, s->g, s->tv, s->rv, s->beta, s->p, s->chol.sb, s->seed, s->ctl, A, kernels,
+                               opt_or(s->opt.no_pdl, 0) == 0));
+  else if (do_beta) CK(beta_solve_launch(s->W, s->Wt, s->g, s->tv, s->beta, s->p, s->seed, s->ctl, A, kernels, opt_or(s->opt.no_pdl, 0) == 0));
   else { CK(beta_keep_launch(s->beta, s->p, s->ctl, A)); *kernels += 1; }
   return HSP_OK;
 }
@@ -183,9 +204,10 @@ static int create_common(hsp_state** out, hsp_state* s) {
   // its own and the pass the rest; otherwise both use every SM and run one after the other.
   const double x_bytes = (double)N * p * (s->dtype == HSP_F32 ? 4.0 : 8.0);
   const double fused_ms_est = x_bytes / 7.0e9 + 0.01;   // the pass streams X at ~7.2 TB/s on B200 (profiles/)
-  CK(chol_plan_create(&s->chol, p, s->num_sms, fused_ms_est));
+  { std::lock_guard<std::mutex> lock(g_opt_mutex); s->opt = g_default_options; }
+  CK(chol_plan_create(&s->chol, p, s->num_sms, fused_ms_est, s->opt));
   const int fused_sms = s->chol.overlap ? s->num_sms - s->chol.K : s->num_sms;
-  s->plan = fused_plan(s->dtype, N, p, fused_sms, s->X);
+  s->plan = fused_plan(s->dtype, N, p, fused_sms, s->X, s->opt);
   s->plan.row_offset = s->row_offset;
   // set opt-in shared-memory attributes now, outside any stream capture
   CK(fused_pass_launch(s->plan, s->X, s->dtype, s->y, -1, p, 0, nullptr, nullptr, nullptr, nullptr, s->stream));
@@ -230,9 +252,8 @@ static int create_common(hsp_state** out, hsp_state* s) {
   // c0: G = X^T X once, by row chunks; with host input the upload of chunk c+1 (copy stream) runs
   // beside the Gram of chunk c
   // fp32 X and a large contraction: tcgen05 tensor cores (split-bf16 products, fp64 flush; ~1e-7 relative);
-  // otherwise exact fp64 DFMA tiles.  HSP_GRAM_TC = 0 / 1 forces the choice.
-  const char* tc_env = getenv("HSP_GRAM_TC");
-  const bool use_tc = s->dtype == HSP_F32 && ((tc_env && *tc_env) ? atoi(tc_env) != 0 : (double)N * p * p >= 2e10);
+  // otherwise exact fp64 DFMA tiles.  Option "gram_tc" = 0 / 1 forces the choice.
+  const bool use_tc = s->dtype == HSP_F32 && (s->opt.gram_tc >= 0 ? s->opt.gram_tc != 0 : (double)N * p * p >= 2e10);
   s->gram_tc = use_tc;
   const GramPlan gp = gram_plan(N, p, s->dtype, s->num_sms, use_tc);
   double* scratch = s->W;                  // W (>= p*p doubles) is free until the first sweep
@@ -265,10 +286,63 @@ static int create_common(hsp_state** out, hsp_state* s) {
   return HSP_OK;
 }
 
+// ---- asynchronous download of the draws (hsp_set_output; "Monte Carlo output is downloaded off of the
+// GPU at the same time as updates for other variables are computed").  The device history of the current call holds
+// rows [0, h_n); after the last sweep of a block of o_block sweeps has been enqueued, an event is recorded on the compute
+// stream, the copy stream waits for it and copies the block's rows of beta, lambda, tau into the host ring, and a second
+// event marks the block as landed.  Nothing here synchronises the host.
+static const size_t kOutEvents = 4096;   // event pairs kept before the oldest is waited for and reused
+
+static int output_flush(hsp_state* s) {
+  if (s->o_cap <= 0 || s->o_pending <= 0) { s->o_pending = 0; return HSP_OK; }
+  const size_t slot = s->o_ev_next % kOutEvents;
+  if (s->o_ev_sweep.size() <= slot) {
+    cudaEvent_t a, b;
+    CK(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+    s->o_ev_sweep.push_back(a); s->o_ev_done.push_back(b); s->o_ev_rows.push_back(0);
+  } else {
+    CK(cudaEventSynchronize(s->o_ev_done[slot]));     // kOutEvents blocks ago; makes the event pair reusable
+    s->o_completed = std::max(s->o_completed, s->o_ev_rows[slot]);
+    s->o_ev_checked = std::max(s->o_ev_checked, s->o_ev_next + 1 - kOutEvents);
+  }
+  CK(cudaEventRecord(s->o_ev_sweep[slot], s->stream));
+  CK(cudaStreamWaitEvent(s->stream3, s->o_ev_sweep[slot], 0));
+  const int p = s->p;
+  long long src = s->o_pending_first, left = s->o_pending;
+  while (left > 0) {
+    const long long dst = s->o_rows % s->o_cap;
+    const long long n = std::min(left, s->o_cap - dst);
+    if (s->o_beta) CK(cudaMemcpyAsync(s->o_beta + (size_t)dst * p, s->h_beta + (size_t)src * p, (size_t)n * p * sizeof(double), cudaMemcpyDeviceToHost, s->stream3));
+    if (s->o_lambda) CK(cudaMemcpyAsync(s->o_lambda + (size_t)dst * p, s->h_lambda + (size_t)src * p, (size_t)n * p * sizeof(double), cudaMemcpyDeviceToHost, s->stream3));
+    if (s->o_tau) CK(cudaMemcpyAsync(s->o_tau + dst, s->h_tau + src, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, s->stream3));
+    s->o_rows += n; src += n; left -= n;
+  }
+  CK(cudaMemcpyAsync(s->h_status, reinterpret_cast<const char*>(s->ctl) + offsetof(Ctl, status), sizeof(int), cudaMemcpyDeviceToHost, s->stream3));
+  CK(cudaEventRecord(s->o_ev_done[slot], s->stream3));
+  s->o_ev_rows[slot] = s->o_rows;
+  s->o_last_done = s->o_ev_done[slot];
+  s->o_ev_next += 1;
+  s->o_pending_first += s->o_pending; s->o_pending = 0;
+  return HSP_OK;
+}
+
+// one more sweep of the current call has been enqueued on the compute stream
+static int output_after_sweep(hsp_state* s, bool last_of_call) {
+  if (s->o_cap <= 0) return HSP_OK;
+  s->o_pending += 1;
+  if (s->o_pending >= s->o_block || last_of_call) return output_flush(s);
+  return HSP_OK;
+}
+
 static int prepare_history(hsp_state* s, long long n_iter) {
   const int p = s->p;
+  // the copy stream may still be reading the history of the previous call: the new call's sweeps start after it
+  if (s->o_last_done) CK(cudaStreamWaitEvent(s->stream, s->o_last_done, 0));
+  s->o_pending_first = 0; s->o_pending = 0;
   if (n_iter > s->h_cap) {
     CK(cudaStreamSynchronize(s->stream));
+    if (s->stream3) CK(cudaStreamSynchronize(s->stream3));
     if (s->h_beta) { cudaFree(s->h_beta); cudaFree(s->h_lambda); cudaFree(s->h_tau); s->h_beta = s->h_lambda = s->h_tau = nullptr; }
     s->h_cap = 0;
     CK(cudaMalloc(&s->h_beta, (size_t)n_iter * p * sizeof(double)));
@@ -284,18 +358,15 @@ static int prepare_history(hsp_state* s, long long n_iter) {
   return HSP_OK;
 }
 
-extern "C" {
-
-const char* hsp_last_error(void) { return g_err.c_str(); }
-
-int hsp_create(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N, int p,
-               unsigned long long seed, void* stream) {
+static int create_device(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N, int p,
+                         unsigned long long seed, long long row_offset, void* stream) {
   if (!out) return fail(HSP_EINVAL, "out is NULL");
   *out = nullptr;
   if (!X || !y) return fail(HSP_EINVAL, "X or y is NULL");
   if (x_dtype != HSP_F32 && x_dtype != HSP_F64) return fail(HSP_EINVAL, "x_dtype must be HSP_F32 or HSP_F64");
   if (N < 2) return fail(HSP_EINVAL, "N must be >= 2");
   if (p < 1) return fail(HSP_EINVAL, "p must be >= 1");
+  if (row_offset < 0) return fail(HSP_EINVAL, "row_offset must be >= 0");
   if (reinterpret_cast<uintptr_t>(X) % (x_dtype == HSP_F32 ? 4 : 8)) return fail(HSP_EINVAL, "X is misaligned");
   cudaPointerAttributes pa{};
   if (cudaPointerGetAttributes(&pa, X) != cudaSuccess || (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)) {
@@ -309,10 +380,19 @@ int hsp_create(hsp_state** out, const void* X, int x_dtype, const unsigned char*
   hsp_state* s = new (std::nothrow) hsp_state();
   if (!s) return fail(HSP_ENOMEM, "out of host memory");
   s->X = X; s->dtype = x_dtype; s->y = y; s->N = N; s->p = p; s->seed = seed; s->stream = (cudaStream_t)stream;
-  s->row_offset = g_pending_row_offset;
+  s->row_offset = row_offset;
   const int rc = create_common(out, s);
   if (rc != HSP_OK) { free_state(s); *out = nullptr; }
   return rc;
+}
+
+extern "C" {
+
+const char* hsp_last_error(void) { return g_err.c_str(); }
+
+int hsp_create(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N, int p,
+               unsigned long long seed, void* stream) {
+  return create_device(out, X, x_dtype, y, N, p, seed, 0, stream);
 }
 
 int hsp_create_host(hsp_state** out, const void* X_host, int x_dtype, const unsigned char* y_host, long long N, int p,
@@ -339,12 +419,7 @@ int hsp_create_host(hsp_state** out, const void* X_host, int x_dtype, const unsi
 
 int hsp_create_shard(hsp_state** out, const void* X, int x_dtype, const unsigned char* y, long long N_local, int p,
                      unsigned long long seed, long long row_offset, void* stream) {
-  if (row_offset < 0) { if (out) *out = nullptr; return fail(HSP_EINVAL, "row_offset must be >= 0"); }
-  // same validation as hsp_create; the offset must be known before the plan is made
-  g_pending_row_offset = row_offset;
-  const int rc = hsp_create(out, X, x_dtype, y, N_local, p, seed, stream);
-  g_pending_row_offset = 0;
-  return rc;
+  return create_device(out, X, x_dtype, y, N_local, p, seed, row_offset, stream);
 }
 
 int hsp_sweep_prepare(hsp_state* s, long long n_iter) {
@@ -360,6 +435,7 @@ int hsp_sweep_begin(hsp_state* s) {
   if (s->split_left <= 0 || s->split_open) return fail(HSP_EINVAL, "hsp_sweep_begin: call hsp_sweep_prepare first / finish the open sweep");
   if (s->flags & HSP_STORE_Z) s->z_valid = !(s->flags & HSP_FREEZE_Z) || s->z_valid;
   else if (!(s->flags & HSP_FREEZE_Z)) s->z_valid = false;
+  if (s->tev_used >= 8192) { CK(cudaStreamSynchronize(s->stream)); const int rc = drain_fused_events(s); if (rc) return rc; }
   long long k = 0;
   const int rc = enqueue_sweep(s, (s->flags & HSP_NO_GRAPH) != 0, &k, 1);
   if (rc != HSP_OK) return rc;
@@ -374,7 +450,7 @@ int hsp_sweep_end(hsp_state* s) {
   const int rc = enqueue_sweep(s, false, &k, 2);
   if (rc != HSP_OK) return rc;
   s->launches += k; s->split_open = false; s->split_left -= 1; s->host_sweep += 1;
-  return HSP_OK;
+  return output_after_sweep(s, s->split_left == 0);
 }
 
 double* hsp_xtz_device(hsp_state* s) { return s ? s->g : nullptr; }
@@ -384,7 +460,103 @@ int hsp_destroy(hsp_state* s) {
   if (!s) return HSP_OK;
   cudaStreamSynchronize(s->stream);
   if (s->stream2) cudaStreamSynchronize(s->stream2);
+  if (s->stream3) cudaStreamSynchronize(s->stream3);
   free_state(s);
+  return HSP_OK;
+}
+
+static int* option_slot(Options& o, const char* key) {
+  struct { const char* name; int Options::*field; } const table[] = {
+      {"fused_eta", &Options::fused_eta}, {"fused_grid", &Options::fused_grid}, {"fused_stages", &Options::fused_stages},
+      {"fused_lag", &Options::fused_lag}, {"fused_w", &Options::fused_w}, {"narrow_rt", &Options::narrow_rt},
+      {"fused_variant", &Options::fused_variant}, {"fused_narrow", &Options::fused_narrow}, {"chol_ctas", &Options::chol_ctas},
+      {"chol_sb", &Options::chol_sb}, {"chol_trace", &Options::chol_trace}, {"gram_tc", &Options::gram_tc},
+      {"no_pdl", &Options::no_pdl}};
+  for (const auto& t : table)
+    if (strcmp(t.name, key) == 0) return &(o.*(t.field));
+  return nullptr;
+}
+
+int hsp_set_option(hsp_state* s, const char* key, long long value) {
+  if (value > 0x7fffffffLL) return fail(HSP_EINVAL, "option value out of range");
+  const int v = value < 0 ? -1 : (int)value;
+  if (s == nullptr) {
+    std::lock_guard<std::mutex> lock(g_opt_mutex);
+    if (key == nullptr) { g_default_options = Options{}; return HSP_OK; }
+    int* slot = option_slot(g_default_options, key);
+    if (!slot) return fail(HSP_EINVAL, std::string("unknown option: ") + key);
+    *slot = v;
+    return HSP_OK;
+  }
+  // an existing chain: its launch plan is fixed; only the launch-mode option can change
+  if (key == nullptr) return fail(HSP_EINVAL, "key is NULL");
+  if (strcmp(key, "no_pdl") != 0) {
+    Options probe;
+    if (!option_slot(probe, key)) return fail(HSP_EINVAL, std::string("unknown option: ") + key);
+    return fail(HSP_EINVAL, std::string("plan-time option (set it with state = NULL before hsp_create): ") + key);
+  }
+  s->opt.no_pdl = v;
+  s->graph_flags = ~0u;        // the captured graph is rebuilt by the next hsp_sweep
+  return HSP_OK;
+}
+
+int hsp_get_option(const hsp_state* s, const char* key, long long* value) {
+  if (!key || !value) return fail(HSP_EINVAL, "NULL argument");
+  Options o;
+  if (s) o = s->opt; else { std::lock_guard<std::mutex> lock(g_opt_mutex); o = g_default_options; }
+  int* slot = option_slot(o, key);
+  if (!slot) return fail(HSP_EINVAL, std::string("unknown option: ") + key);
+  *value = *slot;
+  return HSP_OK;
+}
+
+int hsp_set_output(hsp_state* s, double* host_beta, double* host_lambda, double* host_tau, long long capacity) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  if (capacity < 0) return fail(HSP_EINVAL, "capacity must be >= 0");
+  if (s->split_open) return fail(HSP_EINVAL, "hsp_set_output between hsp_sweep_begin and hsp_sweep_end");
+  // blocks in flight target the old buffers: let them land first
+  if (s->stream3) CK(cudaStreamSynchronize(s->stream3));
+  if (capacity == 0 || (!host_beta && !host_lambda && !host_tau)) {
+    s->o_beta = s->o_lambda = s->o_tau = nullptr; s->o_cap = 0; s->o_rows = 0; s->o_completed = 0; s->o_pending = 0;
+    s->o_ev_checked = s->o_ev_next;
+    return HSP_OK;
+  }
+  if (!s->stream3) CK(cudaStreamCreateWithFlags(&s->stream3, cudaStreamNonBlocking));
+  s->o_beta = host_beta; s->o_lambda = host_lambda; s->o_tau = host_tau; s->o_cap = capacity;
+  s->o_rows = 0; s->o_completed = 0; s->o_pending = 0;
+  s->o_pending_first = s->h_n - s->split_left;        // only sweeps enqueued from now on
+  s->o_ev_checked = s->o_ev_next;
+  // sweeps per download block: at least ~64 KB per block, so that small problems are not bound by copy launches
+  const long long row_bytes = (long long)(2 * s->p + 1) * (long long)sizeof(double);
+  s->o_block = std::max<long long>(1, std::min<long long>((65536 + row_bytes - 1) / row_bytes, std::max<long long>(1, capacity / 2)));
+  return HSP_OK;
+}
+
+int hsp_output_wait(hsp_state* s, long long* rows) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  if (s->o_cap > 0 && s->o_pending > 0) { const int rc = output_flush(s); if (rc != HSP_OK) return rc; }
+  if (s->o_last_done) CK(cudaEventSynchronize(s->o_last_done));
+  s->o_completed = s->o_rows; s->o_ev_checked = s->o_ev_next;
+  if (rows) *rows = s->o_rows;
+  if (s->o_last_done) {
+    if (*s->h_status == HSP_ENOTPD) return fail(HSP_ENOTPD, "Cholesky breakdown: Q is not positive definite");
+    if (*s->h_status == HSP_ENUMERIC) return fail(HSP_ENUMERIC, "non-finite value in the chain state");
+  }
+  return HSP_OK;
+}
+
+int hsp_output_ready(hsp_state* s, long long* rows) {
+  if (!s || !rows) return fail(HSP_EINVAL, "NULL argument");
+  // non-blocking: advance over the blocks whose "landed" event has completed, oldest first
+  while (s->o_ev_checked < s->o_ev_next) {
+    const size_t slot = s->o_ev_checked % kOutEvents;
+    const cudaError_t e = cudaEventQuery(s->o_ev_done[slot]);
+    if (e == cudaErrorNotReady) break;
+    if (e != cudaSuccess) return cuda_fail(e, "cudaEventQuery");
+    s->o_completed = std::max(s->o_completed, s->o_ev_rows[slot]);
+    s->o_ev_checked += 1;
+  }
+  *rows = s->o_completed;
   return HSP_OK;
 }
 
@@ -406,6 +578,7 @@ int hsp_set_flags(hsp_state* s, unsigned flags) {
 int hsp_sweep(hsp_state* s, long long n_iter) {
   if (!s) return fail(HSP_EINVAL, "state is NULL");
   if (n_iter < 0) return fail(HSP_EINVAL, "n_iter must be >= 0");
+  s->split_left = 0; s->split_open = false;
   { const int rc = prepare_history(s, n_iter); if (rc != HSP_OK) return rc; }
   if (n_iter == 0) return HSP_OK;
   if (s->flags & HSP_STORE_Z) s->z_valid = !(s->flags & HSP_FREEZE_Z) || s->z_valid;
@@ -417,13 +590,17 @@ int hsp_sweep(hsp_state* s, long long n_iter) {
       const int rc = enqueue_sweep(s, true, &k);
       if (rc != HSP_OK) return rc;
       s->launches += k;
+      const int rc2 = output_after_sweep(s, it == n_iter - 1); if (rc2 != HSP_OK) return rc2;
     }
   } else {
     if (!s->graph_exec || s->graph_flags != s->flags) {
       const int rc = build_graph(s);
       if (rc != HSP_OK) return rc;
     }
-    for (long long it = 0; it < n_iter; ++it) CK(cudaGraphLaunch(s->graph_exec, s->stream));
+    for (long long it = 0; it < n_iter; ++it) {
+      CK(cudaGraphLaunch(s->graph_exec, s->stream));
+      const int rc2 = output_after_sweep(s, it == n_iter - 1); if (rc2 != HSP_OK) return rc2;
+    }
     s->launches += s->graph_kernels * n_iter;
   }
   s->host_sweep += n_iter;

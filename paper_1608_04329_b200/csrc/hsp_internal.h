@@ -21,6 +21,24 @@ struct Ctl {
 
 enum { kF32 = 0, kF64 = 1 };
 
+// Plan-time options (hsp_set_option, include/hsp.h): -1 = automatic.  A chain copies the process defaults at create.
+struct Options {
+  int fused_eta = -1;      // eta-phase arithmetic for fp32 X: 0 exact fp64, 2 fp32 chains (default)
+  int fused_grid = -1;     // CTAs of the fused pass
+  int fused_stages = -1;   // ring depth S
+  int fused_lag = -1;      // tiles between the eta phase and the x*z phase, D
+  int fused_w = -1;        // compute threads across a row (256 / 512) for rows of 257..512 16-byte vectors
+  int narrow_rt = -1;      // rows per tile of the narrow kernel
+  int fused_variant = -1;  // 0 forces the generic kernel, 1 allows the TMA kernel below 128 vectors per row
+  int fused_narrow = -1;   // 0 disables the narrow kernel
+  int chol_ctas = -1;      // CTAs (SMs) of the Cholesky branch
+  int chol_sb = -1;        // tiles per inverse super-block
+  int chol_trace = -1;     // 1: per-task device timestamps (hsp_dbg_chol_trace)
+  int gram_tc = -1;        // 0 / 1 forces the exact / tensor-core Gram
+  int no_pdl = -1;         // 1: launch the tail kernels without programmatic dependent launch
+};
+inline int opt_or(int v, int dflt) { return v >= 0 ? v : dflt; }
+
 struct FusedPlan {
   int variant;        // 0 = generic, 1 = tma (wide rows), 2 = tma-narrow (width = L lanes per row, chunks = EMAX)
   int grid, block;
@@ -37,7 +55,7 @@ struct FusedPlan {
 };
 
 // ---- fused pass (a1-a3) and reduce (b): fused_pass.cu
-FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X);   // num_sms: CTAs the pass may use
+FusedPlan fused_plan(int dtype, long long N, int p, int num_sms, const void* X, const Options& opt);   // num_sms: CTAs the pass may use
 cudaError_t fused_pass_launch(const FusedPlan& plan, const void* X, int dtype, const unsigned char* y, long long N,
                               int p, unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                               double* z_out, cudaStream_t st);
@@ -87,16 +105,16 @@ struct CholPlan {
 };
 int chol_tiles(int p);                 // nt = ceil(p / 64)
 int chol_ld(int p);                    // P = 64 nt: leading dimension of L, W, Wt (padded with the identity)
-cudaError_t chol_plan_create(CholPlan* plan, int p, int num_sms, double fused_ms_estimate);
+cudaError_t chol_plan_create(CholPlan* plan, int p, int num_sms, double fused_ms_estimate, const Options& opt);
 void chol_plan_destroy(CholPlan* plan);
 cudaError_t cholesky_launch(const CholPlan& plan, const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W,
                             double* Wt, double* Lt, cudaStream_t st, long long* launches);
 cudaError_t beta_solve_launch(const double* W, const double* Wt, const double* g, double* tv, double* beta, int p,
-                              unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches);
+                              unsigned long long seed, Ctl* ctl, cudaStream_t st, long long* launches, bool pdl);
 // block substitution with a block-diagonal inverse (sb < nt); rv: scratch of P doubles
 cudaError_t beta_block_solve_launch(const double* L, const double* Lt, const double* W, const double* Wt, const double* g,
                                     double* tv, double* rv, double* beta, int p, int sb, unsigned long long seed, Ctl* ctl,
-                                    cudaStream_t st, long long* launches);
+                                    cudaStream_t st, long long* launches, bool pdl);
 cudaError_t beta_keep_launch(const double* beta, int p, Ctl* ctl, cudaStream_t st);
 
 // ---- scale conditionals (e1, e2, e3) and draw output (g): scales.cu

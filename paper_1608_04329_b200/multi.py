@@ -1,7 +1,9 @@
-"""Multi-GPU plumbing: one process per GPU, one independent chain per rank
-(seed + rank), no data-path collective.  torch.distributed is used only for the timing reduction and for
-gathering the draws of all chains (convergence diagnostics across chains).  Nothing here touches the
-sampler's arithmetic; it works on any backend (nccl on GPUs, gloo in the CPU tests)."""
+"""Multi-GPU plumbing: one process per GPU, two modes.
+  * independent chains, one per rank (seed + rank): no data-path collective; torch.distributed only reduces the
+    timing and gathers the draws of all chains (cross-chain convergence diagnostics);
+  * ONE chain with the rows of X sharded over the ranks (`sharded_init`, `sharded_sweeps`): one all-reduce of the
+    p x p Gram at init and one all-reduce of X^T z (p doubles) per sweep, issued on the chain's own stream.
+Nothing here touches the sampler's arithmetic; it works on any backend (nccl on GPUs, gloo in the CPU tests)."""
 import torch
 import torch.distributed as dist
 
@@ -66,8 +68,27 @@ def shard_rows(N, rank, world_size):
     return r0, r0 + base + (1 if rank < rem else 0)
 
 
+def _check_stream(chain):
+    """The collective is ordered against the chain's kernels only if both are enqueued on the SAME stream: the chain
+    must have been created on an explicit stream and that stream must be torch's current stream here.  (A chain created
+    without a stream runs on a private stream of the library: the all-reduce would race with reduce_partials and the
+    beta draw.)  Chains that are not CUDA chains (the CPU stand-in of the gloo tests) have no stream_handle."""
+    handle = getattr(chain, "stream_handle", None)
+    if handle is None:
+        return
+    g = chain.xtz_tensor()
+    if not g.is_cuda:
+        return
+    cur = torch.cuda.current_stream(g.device).cuda_stream
+    if handle() == 0 or handle() != cur:
+        raise RuntimeError("row-sharded chain: create the chain with stream=<torch stream> and call sharded_init / "
+                           "sharded_sweeps inside `with torch.cuda.stream(<that stream>)`; chain stream = %#x, current = %#x"
+                           % (handle(), cur))
+
+
 def sharded_init(chain, group=None):
     """Sum the per-shard Gram matrices in place, once (p*p doubles)."""
+    _check_stream(chain)
     if world()[1] > 1:
         dist.all_reduce(chain.gram_tensor(), op=dist.ReduceOp.SUM, group=group)
 
@@ -75,6 +96,7 @@ def sharded_init(chain, group=None):
 def sharded_sweeps(chain, n_iter, group=None):
     """n_iter sweeps of a row-sharded chain: per sweep one all-reduce of X^T z (p doubles) between the local pass
     and the beta draw.  Everything is enqueued on the current stream; there is no host synchronisation."""
+    _check_stream(chain)
     chain.sweep_prepare(n_iter)
     g = chain.xtz_tensor()
     ws = world()[1]

@@ -35,3 +35,12 @@ def mixed_err(got, ref):
     den = np.maximum(np.abs(ref), rms)
     den[den == 0] = 1.0
     return float(np.max(np.abs(got - ref) / den)) if ref.size else 0.0
+
+
+@pytest.fixture
+def hsp_options():
+    """Plan-time options of libhsp.so (hsp_set_option with state NULL) for the chains a test creates; restored after."""
+    import paper_1608_04329_b200 as hsp
+    hsp.reset_options()
+    yield hsp.set_option
+    hsp.reset_options()

@@ -31,6 +31,29 @@ def test_create_rejects_bad_arguments_before_any_device_work():
     assert L.hsp_destroy(None) == 0
 
 
+def test_options_and_output_reject_bad_arguments_without_a_device():
+    """hsp_set_option / hsp_get_option on the process defaults need no GPU; the library reads no environment."""
+    import os
+    hsp.reset_options()
+    assert hsp.get_option("chol_sb") == -1
+    hsp.set_option("chol_sb", 3)
+    assert hsp.get_option("chol_sb") == 3
+    hsp.set_option("chol_sb", -7)                      # any negative value: automatic
+    assert hsp.get_option("chol_sb") == -1
+    L = hsp.lib()
+    assert L.hsp_set_option(None, b"not_an_option", 1) == -1 and b"unknown option" in L.hsp_last_error()
+    v = C.c_longlong()
+    assert L.hsp_get_option(None, None, C.byref(v)) == -1
+    assert L.hsp_set_output(None, None, None, None, 4) == -1
+    assert L.hsp_output_wait(None, None) == -1 and L.hsp_output_ready(None, None) == -1
+    hsp.set_option("gram_tc", 1)
+    hsp.reset_options()
+    assert hsp.get_option("gram_tc") == -1
+    src = "".join(open(os.path.join(os.path.dirname(hsp.lib_path()), "csrc", f)).read()
+                  for f in os.listdir(os.path.join(os.path.dirname(hsp.lib_path()), "csrc")))
+    assert "getenv" not in src
+
+
 def test_binding_is_marshalling_only():
     """The Python package must not contain the method's arithmetic nor reach for the oracle."""
     import inspect

@@ -1,0 +1,50 @@
+"""north_star acceptance "z, beta, lambda, tau agree per iteration over the first 50 sweeps" at the SHAPES of C4 and
+C5 (p = 4000 and p = 2000, fp32 X, the recipes of hsp_synth) with a reduced number of rows so that the oracle's
+O(p^3) sweep stays affordable, through the DEFAULT plan of hsp_create: block substitution with the block-diagonal
+inverse (p > 1280), Cholesky branch serial or beside the pass as the cost model picks.  Also the C5b variant
+(R15: ~5 % positives) and the tightened long-run test."""
+import numpy as np
+import pytest
+import torch
+
+import hsp_synth
+import oracle
+import paper_1608_04329_b200 as hsp
+from conftest import mixed_err
+from test_gpu_parity import run_parity
+
+pytestmark = pytest.mark.gpu
+
+
+def _gram(wl):
+    X64 = wl.X.double()
+    return (X64.T @ X64).cpu().numpy()          # library matmul as the oracle's step 6 input (fp64 definition)
+
+
+def test_c4_shape_p4000_first_50_sweeps():
+    wl = hsp_synth.make("C4", "cuda", n_rows=8009)
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    assert g.fused_variant() == "tma"
+    print("C4 shape plan:", g.plan())
+    g.close()
+    w = run_parity(wl, 50, gram=_gram(wl), check_every=7)
+    assert max(w.values()) < 1e-4
+
+
+def test_c5_shape_p2000_first_50_sweeps():
+    wl = hsp_synth.make("C5", "cuda", n_rows=8009)
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    assert g.fused_variant() == "tma"
+    print("C5 shape plan:", g.plan())
+    g.close()
+    w = run_parity(wl, 50, gram=_gram(wl), check_every=7)
+    assert max(w.values()) < 1e-4
+
+
+def test_c5b_rare_positives_reduced_rows():
+    """C5b: intercept -1.645 sqrt(1 + |beta|^2) gives ~5 % positives (the regime of the paper's real data,
+    PAPER.md:309); the branch-free sampler takes the same path whatever the class balance."""
+    wl = hsp_synth.make("C5b", "cuda", n_rows=8009)
+    assert 0.02 < wl.positive_rate < 0.09
+    w = run_parity(wl, 12, gram=_gram(wl), check_every=3)
+    assert max(w.values()) < 1e-4

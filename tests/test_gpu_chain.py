@@ -77,19 +77,26 @@ def test_beta_conditional_law_on_gpu():
 
 
 def test_long_run_posterior_matches_oracle_c1():
-    """north_star: long-run posterior means and variances agree within 3 Monte-Carlo standard errors
-    (the GPU chain uses a different seed here, so this is a test of the law, not of the coupling)."""
+    """north_star: long-run posterior means and variances agree within 3 Monte-Carlo standard errors (batch means,
+    50 batches; the GPU chain uses a different seed, so this is a test of the law, not of the coupling).  The chains
+    are longer than C1's 2000 sweeps so that the standard errors themselves are well estimated: the second moments of
+    the shrunk null coefficients are heavy-tailed."""
     wl = hsp_synth.make("C1", "cuda")
     Xh, yh = wl.host()
-    o = oracle.OracleChain(Xh, yh, wl.seed); o.sweep(wl.n_sweeps)
-    bo = o.get_draws()[0][500:]
-    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed + 100); g.sweep(4 * wl.n_sweeps)
-    bg = g.get_draws()[0][500:]
+    burn = 1000
+    o = oracle.OracleChain(Xh, yh, wl.seed); o.sweep(3 * wl.n_sweeps + burn)
+    bo = o.get_draws()[0][burn:]
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed + 100); g.sweep(30 * wl.n_sweeps + burn)
+    bg = g.get_draws()[0][burn:]
+    worst = 0.0
     for j in range(wl.p):
-        se = np.hypot(batch_means_se(bo[:, j]), batch_means_se(bg[:, j]))
-        assert abs(bo[:, j].mean() - bg[:, j].mean()) < 3.5 * se + 1e-3, j
+        se = np.hypot(batch_means_se(bo[:, j], 50), batch_means_se(bg[:, j], 50))
+        dm = abs(bo[:, j].mean() - bg[:, j].mean()) / se
         vo, vg = (bo[:, j] - bo[:, j].mean()) ** 2, (bg[:, j] - bg[:, j].mean()) ** 2
-        assert abs(vo.mean() - vg.mean()) < 3.5 * np.hypot(batch_means_se(vo), batch_means_se(vg)) + 1e-4, j
+        dv = abs(vo.mean() - vg.mean()) / np.hypot(batch_means_se(vo, 50), batch_means_se(vg, 50))
+        worst = max(worst, dm, dv)
+        assert dm < 3.0 and dv < 3.0, (j, dm, dv)
+    print("long run C1: worst |difference| / MCSE over", 2 * wl.p, "statistics:", worst)
     # planted truth recovered (PAPER.md:289)
     m = bg.mean(axis=0)
     assert np.all(np.abs(m[:3] - wl.beta_true[:3]) < 0.6) and np.all(np.abs(m[3:]) < 0.12)
@@ -139,3 +146,82 @@ def test_host_entry_with_chunked_upload_matches_device_entry():
     g.sweep(4)
     assert np.array_equal(g.get_draws()[0], b0)
     g.close()
+
+
+@pytest.mark.parametrize("name,n_rows,p,flags", [("C3", 9001, 1000, 0), ("C3", 9001, 1000, hsp.HSP_NO_GRAPH), ("C1", 1000, 10, 0),
+                                                 ("C2", 20011, 100, hsp.HSP_SERIAL)])
+def test_async_output_ring_matches_synchronous_draws(name, n_rows, p, flags):
+    """hsp_set_output (the Monte Carlo output is downloaded while the next updates are computed): the
+    draws that land in the pinned host ring are bit-identical to hsp_get_draws of a chain run synchronously."""
+    wl = hsp_synth.make(name, "cuda", n_rows=n_rows, p=p)
+    n1, n2 = 10, 13
+    (b_ref, l_ref, t_ref), _ = _draws(wl, n1 + n2, flags)
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    g.set_flags(flags)
+    n = n1 + n2
+    hb = torch.zeros((n, p), dtype=torch.float64).pin_memory()
+    hl = torch.zeros((n, p), dtype=torch.float64).pin_memory()
+    ht = torch.zeros(n, dtype=torch.float64).pin_memory()
+    g.set_output(hb, hl, ht, n)
+    g.sweep(n1)
+    g.sweep(n2)                                        # the second call may not overtake the download of the first
+    r0 = g.output_ready()
+    assert 0 <= r0 <= n
+    assert g.output_wait() == n and g.output_ready() == n
+    assert np.array_equal(hb.numpy(), b_ref) and np.array_equal(hl.numpy(), l_ref) and np.array_equal(ht.numpy(), t_ref)
+    # hsp_get_draws still returns the draws of the last call
+    b2, _, t2 = g.get_draws()
+    assert np.array_equal(b2, b_ref[n1:]) and np.array_equal(t2, t_ref[n1:])
+    # a ring smaller than the run keeps the most recent `cap` sweeps at row (r mod cap); beta only
+    cap = 8
+    rb = torch.zeros((cap, p), dtype=torch.float64).pin_memory()
+    g.set_output(rb, None, None, cap)
+    g.sweep(21)
+    assert g.output_wait() == 21
+    b3 = g.get_draws()[0]
+    for r in range(21 - cap, 21):
+        assert np.array_equal(rb.numpy()[r % cap], b3[r]), r
+    # switched off: nothing more is written
+    g.set_output(None, None, None, 0)
+    keep = rb.clone()
+    g.sweep(3)
+    g.sync()
+    assert g.output_wait() == 0 and torch.equal(rb, keep)
+    g.close()
+
+
+def test_async_output_with_sharded_begin_end():
+    wl = hsp_synth.make("C3", "cuda", n_rows=9001)
+    (b_ref, l_ref, t_ref), _ = _draws(wl, 7)
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed, row_offset=0)
+    hb = torch.zeros((7, wl.p), dtype=torch.float64).pin_memory()
+    ht = torch.zeros(7, dtype=torch.float64).pin_memory()
+    g.set_output(hb, None, ht, 7)
+    g.sweep_prepare(7)
+    for _ in range(7):
+        g.sweep_begin(); g.sweep_end()
+    assert g.output_wait() == 7
+    assert np.array_equal(hb.numpy(), b_ref) and np.array_equal(ht.numpy(), t_ref)
+    g.close()
+
+
+def test_options_are_plan_time_and_process_wide(hsp_options):
+    """hsp_set_option: no environment variables; plan-time keys are refused on an existing chain."""
+    wl = hsp_synth.make("C3", "cuda", n_rows=9001)
+    (b_ref, _, _), _ = _draws(wl, 4)
+    hsp_options("fused_variant", 0)
+    assert hsp.get_option("fused_variant") == 0
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    assert g.fused_variant() == "generic"
+    with pytest.raises(hsp.HspError):
+        g.set_option("fused_variant", 1)
+    with pytest.raises(hsp.HspError):
+        hsp.set_option("no_such_key", 1)
+    g.set_option("no_pdl", 1)                          # launch mode: allowed, rebuilds the graph
+    g.sweep(4)
+    b = g.get_draws()[0]
+    g.close()
+    hsp.reset_options()
+    assert hsp.get_option("fused_variant") == -1
+    # generic kernel (exact fp64 eta) vs the TMA kernel (fp32 chains): same chain within the fp32-X tolerance
+    assert np.max(np.abs(b - b_ref)) < 1e-4 * max(1.0, np.max(np.abs(b_ref)))

@@ -72,10 +72,10 @@ def test_c5_shape_tma_f32_p2000_5_sweeps():
 @pytest.mark.parametrize("name,n_rows,p", [("C4", 3001, 4000), ("C4", 777, 3100), ("C5", 1501, 6000), ("C5", 901, 9000),
                                            ("C3", 4099, 640), ("C5", 300, 16000)])
 @pytest.mark.parametrize("eta_mode,z_tol", [(2, 2e-6), (0, 1e-9)])
-def test_fused_pass_only_wide_f32(name, n_rows, p, eta_mode, z_tol, monkeypatch):
+def test_fused_pass_only_wide_f32(name, n_rows, p, eta_mode, z_tol, hsp_options):
     """a1-a3 + b alone (scales and beta frozen at a planted state): z and X^T z against the oracle, in the
     two arithmetic modes of the eta phase (fp32 chains of 4 -> ~2e-7 in z; exact -> ~1e-13)."""
-    monkeypatch.setenv("HSP_FUSED_ETA", str(eta_mode))
+    hsp_options("fused_eta", eta_mode)
     wl = hsp_synth.make(name, "cuda", n_rows=n_rows, p=p)
     Xh, yh = wl.host()
     beta = wl.beta_true * 0.7
@@ -190,10 +190,10 @@ def test_invalid_y_rejected():
 
 
 @pytest.mark.parametrize("sb,p,n_rows", [(2, 333, 3001), (1, 200, 2003), (3, 1000, 4001), (8, 2000, 6001)])
-def test_block_diagonal_inverse_and_block_substitution(sb, p, n_rows, monkeypatch):
+def test_block_diagonal_inverse_and_block_substitution(sb, p, n_rows, hsp_options):
     """d2 by block forward/backward substitution with a block-diagonal inverse (the p > 1280 path), forced at
-    small p through HSP_CHOL_SB: the whole sweep against the oracle."""
-    monkeypatch.setenv("HSP_CHOL_SB", str(sb))
+    small p through the option "chol_sb": the whole sweep against the oracle."""
+    hsp_options("chol_sb", sb)
     wl = hsp_synth.make("C3", "cuda", n_rows=n_rows, p=p)
     X64 = wl.X.double()
     w = run_parity(wl, 6, gram=(X64.T @ X64).cpu().numpy())
@@ -201,11 +201,11 @@ def test_block_diagonal_inverse_and_block_substitution(sb, p, n_rows, monkeypatc
 
 
 @pytest.mark.parametrize("name,n,p", [("C3", 5003, 333), ("C3", 3001, 1000), ("C4", 7001, 520), ("C3", 257, 128), ("C5", 2100, 2000)])
-def test_tensor_core_gram_matches_fp64_definition(name, n, p, monkeypatch):
+def test_tensor_core_gram_matches_fp64_definition(name, n, p, hsp_options):
     """Row c0 on tcgen05 (split-bf16 products, fp32 TMEM accumulation over <= 128 rows, fp64 flush), forced at
     small sizes: against the fp64 definition G = X^T X (library matmul).  The TMEM accumulation truncates: the
     error is a relative bias of about -2e-7; bound 1e-6 of max|G|."""
-    monkeypatch.setenv("HSP_GRAM_TC", "1")
+    hsp_options("gram_tc", 1)
     wl = hsp_synth.make(name, "cuda", n_rows=n, p=p)
     X64 = wl.X.double()
     Go = (X64.T @ X64).cpu().numpy()
@@ -218,3 +218,56 @@ def test_tensor_core_gram_matches_fp64_definition(name, n, p, monkeypatch):
     assert err <= 1e-6
     # and the whole chain on top of it stays inside the fp32-X tolerance
     run_parity(hsp_synth.make(name, "cuda", n_rows=n, p=p), 4, gram=Go)
+
+
+# ---- fused_pass_narrow: every instantiation the default dispatch can reach (fused_pass.cu narrow_plan: EMAX in
+# {4, 6, 8, 12, 16} elements per lane, fp32 chains and exact fp64), whole sweeps against the oracle
+NARROW_CASES = [
+    # config (dtype), rows, p, elements per lane E = ceil(p / 32)
+    ("C3", 12001, 200, 7),    # fp32, EMAX 8
+    ("C3", 9001, 250, 8),     # fp32, EMAX 8
+    ("C3", 6007, 400, 13),    # fp32, EMAX 16
+    ("C3", 5003, 511, 16),    # fp32, EMAX 16, the widest row the narrow kernel takes
+    ("C3", 9001, 180, 6),     # fp32, EMAX 6
+    ("C3", 6007, 300, 10),    # fp32, EMAX 12
+    ("C3", 20011, 100, 4),    # fp32, EMAX 4
+    ("C2", 6007, 150, 5),     # fp64, EMAX 6
+    ("C2", 4001, 250, 8),     # fp64, EMAX 8
+    ("C2", 5003, 190, 6),     # fp64, EMAX 6
+    ("C2", 4001, 280, 9),     # fp64, EMAX 12
+]
+
+
+@pytest.mark.parametrize("name,n_rows,p,E", NARROW_CASES)
+def test_narrow_kernel_every_instantiation_whole_sweeps(name, n_rows, p, E):
+    wl = hsp_synth.make(name, "cuda", n_rows=n_rows, p=p)
+    assert (p + 31) // 32 == E
+    X64 = wl.X.double()
+    probe = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    assert probe.fused_variant() == "tma-narrow"
+    probe.close()
+    w = run_parity(wl, 8, gram=(X64.T @ X64).cpu().numpy())
+    assert w["z"] < (2e-6 if wl.X.dtype == torch.float32 else 1e-9)
+
+
+@pytest.mark.parametrize("name,n_rows,p,E", NARROW_CASES)
+def test_narrow_kernel_fused_pass_only(name, n_rows, p, E):
+    """a1-a3 + b alone at a planted beta (scales and beta frozen): z and X^T z against the oracle."""
+    wl = hsp_synth.make(name, "cuda", n_rows=n_rows + 13, p=p)
+    Xh, yh = wl.host()
+    beta = wl.beta_true * 0.6
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    assert g.fused_variant() == "tma-narrow"
+    g.set_flags(hsp.HSP_STORE_Z | hsp.HSP_FREEZE_SCALES | hsp.HSP_FREEZE_BETA)
+    g.set_state(beta=beta, sweep=11)
+    o = oracle.OracleChain(Xh, yh, wl.seed, gram=np.zeros((p, p)))
+    o.set_flags(oracle.STORE_Z | oracle.FREEZE_SCALES | oracle.FREEZE_BETA)
+    o.set_state(beta=beta, sweep=11)
+    g.sweep(1); o.sweep(1)
+    zg, sg = g.get_latent(); zo, so = o.get_latent()
+    assert np.array_equal(sg, so)
+    ez, eg = mixed_err(zg, zo), mixed_err(g.get_xtz(), o.get_xtz())
+    print(name, n_rows, p, "E", E, "narrow fused pass only: z", ez, "xtz", eg)
+    f32 = wl.X.dtype == torch.float32
+    assert ez < (2e-6 if f32 else 1e-11) and eg < (1e-5 if f32 else 1e-11)
+    g.close()

@@ -22,8 +22,16 @@ def test_single_shard_equals_plain_chain_bitwise():
     b0, l0, t0 = g.get_draws()
     g.close()
     s = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed, row_offset=0)
-    multi.sharded_init(s)
-    multi.sharded_sweeps(s, 6)
+    with pytest.raises(RuntimeError):
+        multi.sharded_sweeps(s, 1)                      # no explicit stream: the collective could not be ordered
+    s.close()
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        s = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed, stream=stream, row_offset=0)
+        multi.sharded_init(s)
+        multi.sharded_sweeps(s, 6)
+    with pytest.raises(RuntimeError):
+        multi.sharded_sweeps(s, 1)                      # called outside the chain's stream
     b, l, t = s.get_draws()
     assert np.array_equal(b, b0) and np.array_equal(l, l0) and np.array_equal(t, t0)
     with pytest.raises(hsp.HspError):

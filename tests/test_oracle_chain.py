@@ -209,3 +209,33 @@ def test_inverse_cdf_and_paper_rejection_give_same_posterior():
         assert abs(ba[:, j].mean() - bc[:, j].mean()) < 4 * se + 2e-3
         va, vc = (ba[:, j] - ba[:, j].mean()) ** 2, (bc[:, j] - bc[:, j].mean()) ** 2
         assert abs(va.mean() - vc.mean()) < 4 * np.hypot(batch_means_se(va), batch_means_se(vc)) + 1e-3
+
+
+def test_row_chunk_mode_matches_default():
+    """The timing-only ROW_CHUNKS mode of the oracle (steps 1-3 over fixed 4096-row chunks on all cores, partials of
+    X^T z added in chunk order; SURVEY.md 8(d) oracle timing (ii)) is the same chain as the default path up to the
+    summation order of g, and does not depend on the number of threads."""
+    import ctypes
+    gomp = ctypes.CDLL("libgomp.so.1")
+    wl = hsp_synth.make("C2", "cpu", n_rows=9001, p=40)
+    Xh, yh = wl.host()
+    ref = oracle.OracleChain(Xh, yh, wl.seed); ref.sweep(6)
+    b0, l0, t0 = ref.get_draws()
+    z0, s0 = ref.get_latent()
+    outs = []
+    n_max = oracle.max_threads()
+    for threads in (1, 3, n_max):
+        gomp.omp_set_num_threads(threads)
+        assert oracle.max_threads() == threads
+        ch = oracle.OracleChain(Xh, yh, wl.seed)
+        ch.set_flags(oracle.STORE_Z | oracle.ROW_CHUNKS)
+        ch.sweep(6)
+        outs.append((ch.get_draws(), ch.get_latent(), ch.get_xtz()))
+    for (b, l, t), (z, s), g in outs:
+        assert np.array_equal(s, s0)
+        assert np.max(np.abs(b - b0)) < 1e-11 and np.max(np.abs(np.log(l / l0))) < 1e-10 and np.max(np.abs(t / t0 - 1)) < 1e-11
+        assert np.max(np.abs(z - z0)) < 1e-10
+    # chunk-ordered reduction: identical whatever the schedule
+    for o in outs[1:]:
+        assert np.array_equal(o[0][0], outs[0][0][0]) and np.array_equal(o[2], outs[0][2])
+    assert oracle.max_threads() >= 1
