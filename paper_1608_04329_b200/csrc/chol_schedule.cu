@@ -6,8 +6,11 @@
 //                                                          i >  j: L_ij = acc W_jj^T
 //   B(i,j), i <  j : acc = - sum_{k=i}^{j-1} L_jk Wt_ik^T ; W_ji = W_jj acc      (same inverse super-block only)
 // A k-loop only needs FRESH data in its last step, so the tiles on the critical path -- the diagonal and
-// the first sub-diagonal of every column -- are split into a prefix task (k < j-1, stores the partial
-// accumulator to a workspace slot) and a short finish task.  Every CTA runs its own list in order and
+// the first sub-diagonal of every column -- are split into a prefix task (stores the partial accumulator to a
+// workspace slot) and a short finish.  With K >= 2 CTAs the finishes are the CHAIN tasks of the first list (a
+// dedicated CTA, operands kept in its shared memory): POTRF(j) (type 2: potrf + inverse of the diagonal tile),
+// TRSM(j) (type 3: L(j+1,j) from the parked accumulator with every k < j applied) and SYRK(j) (type 4: the last
+// update of A(j+1,j+1)); with K = 1 they are ordinary finish tasks of type 0.  Every CTA runs its own list in order and
 // waits on per-tile flags inside a task; the lists are subsequences of one global order in which every
 // producer is placed before its consumers, so with all CTAs co-resident the spin-waits cannot deadlock.
 // The lists come from a greedy list scheduler driven by a cost model of the kernel (microseconds below,
@@ -24,7 +27,7 @@ namespace hsp {
 
 namespace {
 
-struct Cost { double mac = 3.3, hop = 2.0, potrf = 8.0, trinv = 3.0, store = 0.9, loadp = 0.5; };   // us, from HSP_CHOL_TRACE at p = 1000
+struct Cost { double mac = 3.3, hop = 2.0, potrf = 8.0, trinv = 3.0, store = 0.9, loadp = 0.5, cmac = 2.6; };   // us, from the chol_trace option at p = 1000 (cmac: a product of the chain CTA, operands in shared memory)
 
 struct Step { double cost; int dep[2]; };                 // deps are task ids (-1 = none)
 struct Node {
@@ -37,14 +40,51 @@ struct Node {
 
 struct Graph {
   std::vector<Node> n;
+  std::vector<int> chain;                                  // ids of the chain tasks, in execution order
   int n_slots = 0;
 };
 
-Graph build_graph(int nt, int sb, const Cost& c) {
+Graph build_graph(int nt, int sb, const Cost& c, bool chain) {
   Graph g;
   std::vector<int> idL((size_t)nt * nt, -1), idB((size_t)nt * nt, -1);
   auto add = [&](const CholTask& t) { g.n.push_back(Node{t, {}, {}, {}, 0.0, 0.0}); return (int)g.n.size() - 1; };
   // L tiles, column by column (ids increase along a valid topological order)
+  if (chain) {
+    int prev = -1;                                         // previous chain task (same CTA: runs in order)
+    for (int j = 0; j < nt; ++j) {
+      // prefix of the sub-diagonal tile (j+1, j): every k < j;  prefix of the NEXT diagonal tile (j+1, j+1): every k < j
+      int ps = -1, pd = -1, slot_s = -1, slot_d = -1;
+      if (j + 1 < nt && j >= 1) {
+        slot_s = g.n_slots++;
+        ps = add(CholTask{0, j + 1, j, 0, j, -1, slot_s, 0});
+        for (int k = 0; k < j; ++k) g.n[ps].steps.push_back(Step{c.mac, {idL[(size_t)(j + 1) * nt + k], idL[(size_t)j * nt + k]}});
+        g.n[ps].steps.push_back(Step{c.store, {-1, -1}});
+        slot_d = g.n_slots++;
+        pd = add(CholTask{0, j + 1, j + 1, 0, j, -1, slot_d, 0});
+        for (int k = 0; k < j; ++k) g.n[pd].steps.push_back(Step{c.mac, {idL[(size_t)(j + 1) * nt + k], -1}});
+        g.n[pd].steps.push_back(Step{c.store, {-1, -1}});
+      }
+      const int po = add(CholTask{2, j, j, 0, 0, -1, -1, 0});
+      g.n[po].steps.push_back(Step{c.potrf + c.trinv + c.store, {prev, -1}});
+      g.chain.push_back(po); prev = po;
+      idL[(size_t)j * nt + j] = po;
+      if (j + 1 < nt) {
+        const int tr = add(CholTask{3, j + 1, j, 0, 0, slot_s, -1, 0});
+        g.n[tr].steps.push_back(Step{c.loadp + c.cmac + c.store, {po, ps}});
+        g.chain.push_back(tr);
+        idL[(size_t)(j + 1) * nt + j] = tr;
+        const int sy = add(CholTask{4, j + 1, j, 0, 0, slot_d, -1, 0});
+        g.n[sy].steps.push_back(Step{c.loadp + c.cmac, {tr, pd}});
+        g.chain.push_back(sy); prev = sy;
+      }
+      for (int i = j + 2; i < nt; ++i) {
+        const int id = add(CholTask{0, i, j, 0, j, -1, -1, 0});
+        for (int k = 0; k < j; ++k) g.n[id].steps.push_back(Step{c.mac, {idL[(size_t)i * nt + k], idL[(size_t)j * nt + k]}});
+        g.n[id].steps.push_back(Step{c.mac + c.store, {po, -1}});
+        idL[(size_t)i * nt + j] = id;
+      }
+    }
+  } else
   for (int j = 0; j < nt; ++j)
     for (int i = j; i < nt; ++i) {
       const bool split = (i == j || i == j + 1) && j >= 2;

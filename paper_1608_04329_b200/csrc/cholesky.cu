@@ -12,8 +12,12 @@
 //   L(i,j), i >= j :  A = Q_ij - sum_{k<j} L_ik L_jk^T ;  i == j: L_jj = chol(A), W_jj = L_jj^-1 ;
 //                                                         i >  j: L_ij = A W_jj^T
 //   B(i,j), i <  j :  A = - sum_{k=i}^{j-1} L_jk Wt_ik^T ; W_ji = W_jj A  (stored in W and, transposed, in Wt)
-// The host (chol_schedule.cu) splits the tiles on the critical path into prefix + finish tasks and deals all
-// tasks to the CTAs as static ordered lists; a CTA runs its list in order and waits on per-tile "done" flags
+// The critical path of the factorisation is  potrf(j) -> L(j+1,j) = A W_jj^T -> A(j+1,j+1) -= L(j+1,j) L(j+1,j)^T ->
+// potrf(j+1): with two or more CTAs it is run by ONE dedicated CTA (the first list) as three chain tasks per column
+// whose operands stay in its shared memory (types 2, 3, 4 below) -- no flag round trips through global memory between
+// them; all other CTAs feed it partial accumulators (prefix tasks) and take the bulk of the products.  With a single
+// CTA the host (chol_schedule.cu) instead splits the tiles on the critical path into prefix + finish tasks.  All
+// tasks are dealt to the CTAs as static ordered lists; a CTA runs its list in order and waits on per-tile "done" flags
 // inside the k-loop.  All CTAs are co-resident (cooperative launch) and every list is a subsequence of one
 // global order in which producers precede consumers, so the spin-waits cannot deadlock.  Every tile is
 // accumulated in ascending k by a fixed sequence of tasks: the result does not depend on the number of CTAs.
@@ -296,10 +300,113 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
   int* fP = fB + (size_t)nt * nt;
   const double tau_inv2 = ctl->tau_inv2;
 
+  // c: the Q tile (ti, tj) in the accumulator layout, padded with the identity
+  auto load_q_tile = [&](int ti_, int tj_, double (&a)[4][2][2]) {
+#pragma unroll
+    for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          double v = 0.0;
+          const int gr = ti_ * CT + f.row0 + mb * 8 + f.g, gc = tj_ * CT + f.col0 + nb * 8 + 2 * f.t + e;
+          if (gr < p && gc < p) {
+            v = G[(size_t)gr * p + gc];
+            if (gr == gc) v = fma(tau_inv2, lam_inv2[gr], v);
+          } else if (gr == gc) v = 1.0;
+          a[mb][nb][e] = v;
+        }
+  };
+  auto load_slot = [&](int slot, double (&a)[4][2][2]) {
+    wait_flag(&fP[slot]);
+    const double2* src = reinterpret_cast<const double2*>(ws + (size_t)slot * CT * CT);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const double2 v = __ldcg(src + q * kCholThreads + tid);
+      a[q >> 1][q & 1][0] = v.x; a[q >> 1][q & 1][1] = v.y;
+    }
+  };
+  auto acc_to_smem = [&](const double (&a)[4][2][2], double* T) {
+#pragma unroll
+    for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb)
+        *reinterpret_cast<double2*>(T + (f.row0 + mb * 8 + f.g) * TLD + f.col0 + nb * 8 + 2 * f.t) = make_double2(a[mb][nb][0], a[mb][nb][1]);
+  };
+  // diagonal tile: L_jj = chol(S), W_jj = L_jj^-1 (X), both written out (with Wt and, if asked for, Lt); flag released
+  auto diag_finish = [&](int j_) {
+    const bool ok = tile_potrf(S, rdiag, tid);
+    if (!ok && tid == 0) atomicCAS(&ctl->status, 0, -4);
+    tile_trinv(S, rdiag, X, tid);
+    for (int e = tid; e < CT * CT / 2; e += kCholThreads) {
+      const int r = e / (CT / 2), c = (e % (CT / 2)) * 2;
+      const size_t g = (size_t)(j_ * CT + r) * P + j_ * CT + c;
+      double2 l = *reinterpret_cast<const double2*>(S + r * TLD + c);
+      if (c > r) l.x = 0.0;
+      if (c + 1 > r) l.y = 0.0;
+      *reinterpret_cast<double2*>(L + g) = l;
+      *reinterpret_cast<double2*>(W + g) = *reinterpret_cast<const double2*>(X + r * TLD + c);
+      *reinterpret_cast<double2*>(Wt + g) = make_double2(X[c * TLD + r], X[(c + 1) * TLD + r]);
+      if (Lt != nullptr)   // L^T, used by the block back-substitution when only a block-diagonal inverse is built
+        *reinterpret_cast<double2*>(Lt + g) = make_double2(c >= r ? S[c * TLD + r] : 0.0, c + 1 >= r ? S[(c + 1) * TLD + r] : 0.0);
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) st_release(&fL[(size_t)j_ * nt + j_], 1);
+  };
+
   const int t_end = list_off[blockIdx.x + 1];
   for (int ti = list_off[blockIdx.x]; ti < t_end; ++ti) {
     const CholTask tk = tasks[ti];
     if (trace != nullptr && tid == 0) trace[4 * (size_t)ti] = globaltimer_ns();
+    if (tk.type >= 2) {
+      // ---- chain tasks (dedicated CTA; S, X persist in shared memory from one chain task to the next)
+      const int j = tk.j;
+      double acc[4][2][2];
+      if (tk.type == 2) {
+        // POTRF(j): S holds A_jj (left there by SYRK(j-1); column 0: the Q tile)
+        if (j == 0) { load_q_tile(0, 0, acc); acc_to_smem(acc, S); }
+        __syncthreads();
+        diag_finish(j);
+      } else if (tk.type == 3) {
+        // TRSM(j): L(j+1,j) = A W_jj^T, A = parked accumulator of (j+1,j) with every k < j applied (column 0: Q tile);
+        // W_jj is still in X.  The product goes to global memory and stays in S as the operand of SYRK(j).
+        if (tk.slot_in >= 0) load_slot(tk.slot_in, acc); else load_q_tile(j + 1, j, acc);
+        __syncthreads();                              // everyone is done with S (L_jj was written out by POTRF(j))
+        acc_to_smem(acc, S);
+        __syncthreads();
+        double out[4][2][2];
+#pragma unroll
+        for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+          for (int nb = 0; nb < 2; ++nb) out[mb][nb][0] = out[mb][nb][1] = 0.0;
+        tile_mma<TLD, TLD, CT, false>(S, X, f, out);
+#pragma unroll
+        for (int mb = 0; mb < 4; ++mb)
+#pragma unroll
+          for (int nb = 0; nb < 2; ++nb) {
+            const int r = (j + 1) * CT + f.row0 + mb * 8 + f.g, c = j * CT + f.col0 + nb * 8 + 2 * f.t;
+            *reinterpret_cast<double2*>(L + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
+            if (Lt != nullptr) { Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1]; }
+          }
+        __syncthreads();                              // the product has been read from S by every warp
+        acc_to_smem(out, S);
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) st_release(&fL[(size_t)(j + 1) * nt + j], 1);
+      } else {
+        // SYRK(j): A(j+1,j+1) = parked accumulator (every k < j applied; column 1: Q tile) - L(j+1,j) L(j+1,j)^T -> S
+        if (tk.slot_in >= 0) load_slot(tk.slot_in, acc); else load_q_tile(j + 1, j + 1, acc);
+        tile_mma<TLD, TLD, CT, true>(S, S, f, acc);
+        __syncthreads();
+        acc_to_smem(acc, S);
+      }
+      if (trace != nullptr && tid == 0) {
+        const unsigned long long tn = globaltimer_ns();
+        trace[4 * (size_t)ti + 1] = tn; trace[4 * (size_t)ti + 2] = tn; trace[4 * (size_t)ti + 3] = blockIdx.x;
+      }
+      continue;
+    }
     const bool isL = tk.type == 0;
     const int i = tk.i, j = tk.j;
     // operands of the k loop: acc -= MA(ra,k) MB(rb,k)^T
@@ -309,31 +416,13 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
     const int kbeg = tk.kbeg, kend = tk.kend;
 
     double acc[4][2][2];
-    if (tk.slot_in >= 0) {
-      wait_flag(&fP[tk.slot_in]);
-      const double2* src = reinterpret_cast<const double2*>(ws + (size_t)tk.slot_in * CT * CT);
-#pragma unroll
-      for (int q = 0; q < 8; ++q) {
-        const double2 v = __ldcg(src + q * kCholThreads + tid);
-        acc[q >> 1][q & 1][0] = v.x; acc[q >> 1][q & 1][1] = v.y;
-      }
-    } else {
+    if (tk.slot_in >= 0) load_slot(tk.slot_in, acc);
+    else if (isL) load_q_tile(i, j, acc);
+    else {
 #pragma unroll
       for (int mb = 0; mb < 4; ++mb)
 #pragma unroll
-        for (int nb = 0; nb < 2; ++nb)
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            double v = 0.0;
-            if (isL) {                               // c: Q tile, padded with the identity
-              const int gr = i * CT + f.row0 + mb * 8 + f.g, gc = j * CT + f.col0 + nb * 8 + 2 * f.t + e;
-              if (gr < p && gc < p) {
-                v = G[(size_t)gr * p + gc];
-                if (gr == gc) v = fma(tau_inv2, lam_inv2[gr], v);
-              } else if (gr == gc) v = 1.0;
-            }
-            acc[mb][nb][e] = v;
-          }
+        for (int nb = 0; nb < 2; ++nb) acc[mb][nb][0] = acc[mb][nb][1] = 0.0;
     }
 
     const int nchunks = (kend - kbeg) * (CT / KC);
@@ -381,31 +470,9 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       if (tid == 0) st_release(&fP[tk.slot_out], 1);
     } else if (isL && i == j) {
       // ---- diagonal: L_jj = chol(acc), W_jj = L_jj^-1
-#pragma unroll
-      for (int mb = 0; mb < 4; ++mb)
-#pragma unroll
-        for (int nb = 0; nb < 2; ++nb)
-          *reinterpret_cast<double2*>(S + (f.row0 + mb * 8 + f.g) * TLD + f.col0 + nb * 8 + 2 * f.t) =
-              make_double2(acc[mb][nb][0], acc[mb][nb][1]);
+      acc_to_smem(acc, S);
       __syncthreads();
-      const bool ok = tile_potrf(S, rdiag, tid);
-      if (!ok && tid == 0) atomicCAS(&ctl->status, 0, -4);
-      tile_trinv(S, rdiag, X, tid);
-      for (int e = tid; e < CT * CT / 2; e += kCholThreads) {
-        const int r = e / (CT / 2), c = (e % (CT / 2)) * 2;
-        const size_t g = (size_t)(j * CT + r) * P + j * CT + c;
-        double2 l = *reinterpret_cast<const double2*>(S + r * TLD + c);
-        if (c > r) l.x = 0.0;
-        if (c + 1 > r) l.y = 0.0;
-        *reinterpret_cast<double2*>(L + g) = l;
-        *reinterpret_cast<double2*>(W + g) = *reinterpret_cast<const double2*>(X + r * TLD + c);
-        *reinterpret_cast<double2*>(Wt + g) = make_double2(X[c * TLD + r], X[(c + 1) * TLD + r]);
-        if (Lt != nullptr)   // L^T, used by the block back-substitution when only a block-diagonal inverse is built
-          *reinterpret_cast<double2*>(Lt + g) = make_double2(c >= r ? S[c * TLD + r] : 0.0, c + 1 >= r ? S[(c + 1) * TLD + r] : 0.0);
-      }
-      __threadfence();
-      __syncthreads();
-      if (tid == 0) st_release(&fL[(size_t)j * nt + j], 1);
+      diag_finish(j);
     } else {
       // ---- off-diagonal: multiply by W_jj (from global; written by the diagonal task of column j)
       wait_flag(&fL[(size_t)j * nt + j]);
@@ -665,7 +732,10 @@ cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_e
     // the cost model is calibrated with the factor's working set in L2; when G, L, Lt (or W, Wt) do not fit beside
     // the X stream (p >= ~1500) the tile loads of the overlapped branch go to HBM: measured ~1.3x at p = 2000
     const double ws_mb = 3.0 * (double)pl->P * pl->P * 8.0 / 1e6;
-    const double budget_us = 0.85 * fused_ms_estimate * 1e3 / (ws_mb > 48.0 ? 1.3 : 1.0);
+    // 0.70: the branch is latency-bound and slows down with the SM clock, the HBM-bound pass does not -- under the
+    // board's power cap (~1.5-1.7 GHz instead of 1.965) a branch sized to 85 % of the pass became the critical path
+    // (C3, 1000 sweeps: 1699 sweeps/s with 16 SMs, 1731 with 20)
+    const double budget_us = 0.70 * fused_ms_estimate * 1e3 / (ws_mb > 48.0 ? 1.3 : 1.0);
     const int cands[] = {2, 4, 6, 8, 10, 12, 16, 20, 24, 32, 40, 48};
     bool found = false;
     if (nt <= 40)

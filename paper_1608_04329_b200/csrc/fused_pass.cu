@@ -114,44 +114,76 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
 // ------------------------------------------------------------------------------------------------
 // Column-stripe arithmetic for one 16-byte vector of X
 // ------------------------------------------------------------------------------------------------
+// Packed fp32 pairs (sm_100: fma.rn.f32x2 -> SASS FFMA2, two fp32 FMAs per issued instruction; each half is an
+// ordinary IEEE fp32 FMA).  Halves the FMA instruction count of the fp32-X phases.
+__device__ __forceinline__ unsigned long long f2_pack(float a, float b) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b));
+  return r;
+}
+__device__ __forceinline__ void f2_unpack(unsigned long long v, float& a, float& b) {
+  asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ void ld_shared_b64x2(uint32_t a, unsigned long long& lo, unsigned long long& hi) {
+  asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(lo), "=l"(hi) : "r"(a));
+}
+
 template <typename XT> struct Vec;
 template <> struct Vec<float> {
   static constexpr int V = 4;
   using Acc = float;
-  float4 v;
-  __device__ __forceinline__ void load(uint32_t smem_addr) { v = ld_shared_f32x4(smem_addr); }
+  using Pair = unsigned long long;          // accumulators of a 16-byte vector: two packed fp32 pairs
+  unsigned long long lo, hi;                // (x0, x1), (x2, x3)
+  __device__ __forceinline__ void load(uint32_t smem_addr) { ld_shared_b64x2(smem_addr, lo, hi); }
   __device__ __forceinline__ double dot(const double* b) const {
-    double s = (double)v.x * b[0];
-    s = fma((double)v.y, b[1], s);
-    s = fma((double)v.z, b[2], s);
-    s = fma((double)v.w, b[3], s);
+    float x0, x1, x2, x3;
+    f2_unpack(lo, x0, x1); f2_unpack(hi, x2, x3);
+    double s = (double)x0 * b[0];
+    s = fma((double)x1, b[1], s);
+    s = fma((double)x2, b[2], s);
+    s = fma((double)x3, b[3], s);
     return s;
   }
-  // fp32 chain of 4 (eta modes 1, 2): at most 4 roundings of 2^-24 relative to the running partial
-  __device__ __forceinline__ float dotf(const float* b) const {
-    float s = v.x * b[0];
-    s = fmaf(v.y, b[1], s);
-    s = fmaf(v.z, b[2], s);
-    s = fmaf(v.w, b[3], s);
-    return s;
+  // fp32 (eta mode 2): part += x .* b on packed pairs; the two halves are two chains of 2 FMAs per vector, added at
+  // the end of the row's chunks -- at most ~2C+1 roundings of 2^-24 relative to the running partial
+  __device__ __forceinline__ void dotf2(const Pair* b2, Pair& part) const {
+    part = f2_fma(lo, b2[0], part);
+    part = f2_fma(hi, b2[1], part);
   }
-  __device__ __forceinline__ void axpy(float z, float* acc) const {
-    acc[0] = fmaf(v.x, z, acc[0]);
-    acc[1] = fmaf(v.y, z, acc[1]);
-    acc[2] = fmaf(v.z, z, acc[2]);
-    acc[3] = fmaf(v.w, z, acc[3]);
+  __device__ __forceinline__ void axpy(float z, Pair* acc) const {
+    const Pair z2 = f2_pack(z, z);
+    acc[0] = f2_fma(lo, z2, acc[0]);
+    acc[1] = f2_fma(hi, z2, acc[1]);
+  }
+  static __device__ __forceinline__ Pair zero() { return 0ull; }
+  static __device__ __forceinline__ void flush(Pair* acc, double* acc64) {   // acc64[0..3] += acc; acc = 0
+    float a, b;
+    f2_unpack(acc[0], a, b); acc64[0] += (double)a; acc64[1] += (double)b;
+    f2_unpack(acc[1], a, b); acc64[2] += (double)a; acc64[3] += (double)b;
+    acc[0] = acc[1] = 0ull;
   }
 };
 template <> struct Vec<double> {
   static constexpr int V = 2;
   using Acc = double;
+  using Pair = double;
   double2 v;
   __device__ __forceinline__ void load(uint32_t smem_addr) { v = ld_shared_f64x2(smem_addr); }
   __device__ __forceinline__ double dot(const double* b) const { return fma(v.y, b[1], v.x * b[0]); }
-  __device__ __forceinline__ float dotf(const float*) const { return 0.f; }   // never used: fp64 X is always eta mode 0
-  __device__ __forceinline__ void axpy(double z, double* acc) const {
+  __device__ __forceinline__ void dotf2(const Pair*, Pair&) const {}   // never used: fp64 X is always eta mode 0
+  __device__ __forceinline__ void axpy(double z, Pair* acc) const {
     acc[0] = fma(v.x, z, acc[0]);
     acc[1] = fma(v.y, z, acc[1]);
+  }
+  static __device__ __forceinline__ Pair zero() { return 0.0; }
+  static __device__ __forceinline__ void flush(Pair* acc, double* acc64) {
+    acc64[0] += acc[0]; acc64[1] += acc[1];
+    acc[0] = acc[1] = 0.0;
   }
 };
 
@@ -325,22 +357,30 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
     // Stripes past p read column 0 with beta = 0 and are never written back, so the loops below are
     // straight-line code.  All shared-memory addresses are 32-bit and advance incrementally with the ring.
     const int grp = tid / W, wg = (tid % W) >> 5, gt = tid % W;
+    using Pair = typename Vec<XT>::Pair;
     double breg[EM == 0 ? C : 1][V];
-    float bregf[EM == 0 ? 1 : C][V];
+    Pair breg2[EM == 0 ? 1 : C][2];               // beta as packed fp32 pairs (eta mode 2)
     double acc64[C][V];
-    Acc acc[C][V];
+    Pair acc[C][2];
     uint32_t coff[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) {
       const int col = (c * W + gt) * V;
       coff[c] = (col < p) ? (uint32_t)(col * sizeof(XT)) : 0u;
+      double bv[V];
 #pragma unroll
       for (int v = 0; v < V; ++v) {
-        const double bv = (col + v < p) ? beta[col + v] : 0.0;
-        if constexpr (EM == 0) breg[c][v] = bv; else bregf[c][v] = (float)bv;
+        bv[v] = (col + v < p) ? beta[col + v] : 0.0;
         acc64[c][v] = 0.0;
-        acc[c][v] = (Acc)0;
       }
+      if constexpr (EM == 0) {
+#pragma unroll
+        for (int v = 0; v < V; ++v) breg[c][v] = bv[v];
+      } else if constexpr (kF32) {
+        breg2[c][0] = f2_pack((float)bv[0], (float)bv[1]);
+        breg2[c][1] = f2_pack((float)bv[2], (float)bv[3]);
+      }
+      acc[c][0] = acc[c][1] = Vec<XT>::zero();
     }
     const int my_row = grp * RG + row_of_lane<RG>(lane);
     const bool writer = (lane & (32 / RG - 1)) == 0;
@@ -374,15 +414,27 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
           tot = warp_reduce_rows<double, RG>(part, lane);
         } else {
           float part[RG];
+          if constexpr (kF32) {
+            Pair part2[RG];
 #pragma unroll
-          for (int r = 0; r < RG; ++r) part[r] = 0.f;
+            for (int r = 0; r < RG; ++r) part2[r] = 0ull;
 #pragma unroll
-          for (int c = 0; c < C; ++c) {
-            Vec<XT> x[RG];
+            for (int c = 0; c < C; ++c) {
+              Vec<XT> x[RG];
 #pragma unroll
-            for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
+              for (int r = 0; r < RG; ++r) x[r].load(tile + r * rb + coff[c]);
 #pragma unroll
-            for (int r = 0; r < RG; ++r) part[r] += x[r].dotf(bregf[c]);
+              for (int r = 0; r < RG; ++r) x[r].dotf2(breg2[c], part2[r]);
+            }
+#pragma unroll
+            for (int r = 0; r < RG; ++r) {
+              float a, b;
+              f2_unpack(part2[r], a, b);
+              part[r] = a + b;
+            }
+          } else {
+#pragma unroll
+            for (int r = 0; r < RG; ++r) part[r] = 0.f;
           }
           tot = (double)warp_reduce_rows<float, RG>(part, lane);
         }
@@ -434,9 +486,7 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
         if (rows_since_flush >= kFlushRows) {
           rows_since_flush = 0;
 #pragma unroll
-          for (int c = 0; c < C; ++c)
-#pragma unroll
-            for (int v = 0; v < V; ++v) { acc64[c][v] += (double)acc[c][v]; acc[c][v] = (Acc)0; }
+          for (int c = 0; c < C; ++c) Vec<XT>::flush(acc[c], acc64[c]);
         }
       }
     };
@@ -475,9 +525,10 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
 #pragma unroll
     for (int c = 0; c < C; ++c) {
       const int col = (c * W + gt) * V;
+      Vec<XT>::flush(acc[c], acc64[c]);
 #pragma unroll
       for (int v = 0; v < V; ++v)
-        if (col + v < p) partial[((size_t)cta * G + grp) * p + col + v] = acc64[c][v] + (double)acc[c][v];
+        if (col + v < p) partial[((size_t)cta * G + grp) * p + col + v] = acc64[c][v];
     }
   }
 }
@@ -485,36 +536,43 @@ fused_pass_tma(const XT* __restrict__ X, const unsigned char* __restrict__ y, lo
 // ------------------------------------------------------------------------------------------------
 // Narrow rows (fewer than 128 16-byte vectors per row, any p: the rows need not be a multiple of 16 bytes --
 // config C2, and the shape of the paper's real-data run, N = 1.3e6, p = 141).
-// Same pipeline as fused_pass_tma (producer / 16 compute warps / sampler warps, S-stage ring, lag D), but a tile
-// holds RT = 32..256 whole rows (RT a multiple of 32, so a tile starts 16-byte aligned and is a whole number of
-// 16-byte units) and the thread mappings differ:
-//   eta phase   L = 2^k lanes share a row (E = ceil(p / L) <= EMAX elements per lane, beta in registers); the
-//               512 compute threads cover 512/L rows per pass; shuffle reduction over the L lanes.
-//   xz phase    thread t owns column t mod p for the rows r = t div p (mod NG), NG = floor(512 / p) row groups;
-//               the NG accumulators of a column are combined through shared memory at the end (fixed order).
-//   sampler     a sampler warp takes a whole tile: lane = row, RT/32 batches.
-// The ragged last tile may not be a multiple of 16 bytes: the producer copies the 16-byte units by TMA and the
-// last < 16 bytes with plain loads.
+// A tile holds RT = 32..256 whole rows (RT a multiple of 32, so a tile starts 128-byte aligned and the batches of 32
+// rows a z-warp takes never straddle a tile); one cp.async.bulk per tile, S-stage ring.  Warp roles:
+//   producer   1 thread: streams the tiles (the < 16 trailing bytes of a ragged last tile by plain loads).
+//   z-warps    8 warps, batches of 32 rows dealt round-robin (lane = row): eta_i = x_i . beta by a THREAD-PER-ROW dot
+//              product straight from the tile in shared memory (beta staged once in shared memory, read as 16-byte
+//              broadcasts), then the Philox uniform and TNpos -> z to shared memory.  No shuffles, no eta round trip.
+//              Bank conflicts: lanes read the same column of 32 consecutive rows, i.e. addresses row_bytes apart.  With
+//              U = the largest power of two <= 16 that divides row_bytes, the row is read in U-byte units; row_bytes / U
+//              is odd for U < 16, which makes the 4-, 8-byte accesses of a warp conflict-free; for U = 16 and
+//              q = row_bytes / 16 even, lane r of each quarter-warp starts (r >> shift) units later (and wraps), which
+//              spreads the 8 lanes over the 8 16-byte banks again (shift = log2(8 / gcd(q, 8))).
+//   x*z warps  16 warps: thread t owns column t mod p for the rows t div p (mod NG), NG = floor(512 / p); conflict-free
+//              4-/8-byte loads along the row; the NG accumulators of a column are combined through shared memory at
+//              the end (fixed order).  fp32 X: fp32 FMA chains, flushed into fp64 every >= 16 rows.
+// Per element of X this is ~2.3 + ~2.6 issued thread-instructions (the previous lane-group/shuffle design: ~7), which is
+// what takes the kernel from issue-bound to HBM-bound at p ~ 100-150.
 // ------------------------------------------------------------------------------------------------
-constexpr int kNarrowSamplers = 8;
-constexpr int kNarrowThreads = (kComputeWarpsAll + kNarrowSamplers + 1) * 32;   // 800
+constexpr int kNarrowZWarps = 8;
+constexpr int kNarrowThreads = (kComputeWarpsAll + kNarrowZWarps + 1) * 32;   // 800
+constexpr int kNarrowMaxP = kComputeThreadsAll - 1;                          // 511: one x*z thread per column
+constexpr size_t kNarrowBetaBytes = (size_t)(kComputeThreadsAll + 16) * sizeof(double);
 
 struct NarrowSmemLayout {
-  size_t tiles, eta, z64, z32, red, bars, total;
-  __host__ __device__ NarrowSmemLayout(int S, int RT, int p, size_t stage_bytes) {
+  size_t tiles, beta, z64, z32, red, bars, total;
+  __host__ __device__ NarrowSmemLayout(int S, int RT, size_t stage_bytes) {
     tiles = 0;
-    eta = tiles + (size_t)S * stage_bytes;
-    z64 = eta + (size_t)S * RT * sizeof(double);
+    beta = tiles + (size_t)S * stage_bytes;
+    z64 = beta + kNarrowBetaBytes;
     z32 = z64 + (size_t)S * RT * sizeof(double);
     red = (z32 + (size_t)S * RT * sizeof(float) + 15) & ~(size_t)15;
     bars = red + (size_t)kComputeThreadsAll * sizeof(double);
-    total = bars + (size_t)4 * S * sizeof(uint64_t);
-    (void)p;
+    total = bars + (size_t)3 * S * sizeof(uint64_t);
   }
 };
 
-// A stage is RT rows plus 1 KB that TMA never writes and that stays zero: the eta phase reads up to EMAX L - p
-// elements past the end of a row (times beta = 0), which for the last row of a tile lands in this pad.
+// A stage is RT rows plus 1 KB that TMA never writes and that stays zero: the last 16-byte step of a row's dot product
+// may read up to 12 bytes past the end of the row (times beta = 0), which for the last row of a tile lands in this pad.
 __host__ __device__ constexpr size_t narrow_stage_bytes(int RT, size_t row_bytes) {
   return (((size_t)RT * row_bytes + 127) & ~(size_t)127) + 1024;
 }
@@ -523,39 +581,119 @@ template <typename XT> __device__ __forceinline__ XT ld_shared_x(uint32_t a);
 template <> __device__ __forceinline__ float ld_shared_x<float>(uint32_t a) { return ld_shared_f32(a); }
 template <> __device__ __forceinline__ double ld_shared_x<double>(uint32_t a) { return ld_shared_f64(a); }
 
-template <typename XT, int EMAX, int EM>
+// 16 bytes of a row, read in U-byte units (U = 4, 8, 16)
+template <int U> __device__ __forceinline__ float4 ld_step_f32(uint32_t a) {
+  if constexpr (U == 16) return ld_shared_f32x4(a);
+  else if constexpr (U == 8) {
+    const float2 lo = ld_shared_f32x2(a), hi = ld_shared_f32x2(a + 8);
+    return make_float4(lo.x, lo.y, hi.x, hi.y);
+  } else return make_float4(ld_shared_f32(a), ld_shared_f32(a + 4), ld_shared_f32(a + 8), ld_shared_f32(a + 12));
+}
+template <int U> __device__ __forceinline__ double2 ld_step_f64(uint32_t a) {
+  if constexpr (U == 16) return ld_shared_f64x2(a);
+  else return make_double2(ld_shared_f64(a), ld_shared_f64(a + 8));
+}
+
+// eta of one row: sum over n_steps 16-byte steps of the row at shared address xrow; beta0: beta in shared memory in
+// the accumulation type (float for fp32 X with EM != 0, else double), zero beyond p.  delta: start offset (in steps) of
+// this lane for U = 16 (see above), 0 otherwise.
+template <typename XT, int U, int EM>
+__device__ __forceinline__ double narrow_row_dot(uint32_t xrow, uint32_t beta0, int n_steps, int delta) {
+  constexpr bool kF32 = sizeof(XT) == 4;
+  auto rot = [&](int c) {
+    if constexpr (U == 16) { c += delta; c = c >= n_steps ? c - n_steps : c; }
+    return c;
+  };
+  if constexpr (kF32 && EM != 0) {
+    // fp32 chains of <= 16 FMAs per accumulator (4 accumulators = the 4 elements of a step, as two packed pairs:
+    // FFMA2), flushed into fp64
+    double eta = 0.0;
+    for (int c0 = 0; c0 < n_steps; c0 += 16) {
+      const int c1 = c0 + 16 < n_steps ? c0 + 16 : n_steps;
+      unsigned long long a01 = 0ull, a23 = 0ull;
+#pragma unroll 4
+      for (int c = c0; c < c1; ++c) {
+        const uint32_t off = (uint32_t)rot(c) * 16u;
+        unsigned long long b01, b23, x01, x23;
+        ld_shared_b64x2(beta0 + off, b01, b23);
+        if constexpr (U == 16) ld_shared_b64x2(xrow + off, x01, x23);
+        else {
+          const float4 x = ld_step_f32<U>(xrow + off);
+          x01 = f2_pack(x.x, x.y); x23 = f2_pack(x.z, x.w);
+        }
+        a01 = f2_fma(x01, b01, a01); a23 = f2_fma(x23, b23, a23);
+      }
+      float a0, a1, a2, a3;
+      f2_unpack(a01, a0, a1); f2_unpack(a23, a2, a3);
+      eta += ((double)a0 + (double)a1) + ((double)a2 + (double)a3);
+    }
+    return eta;
+  } else if constexpr (kF32) {
+    // exact: every element converted to fp64 (beta: 4 doubles per step)
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+#pragma unroll 2
+    for (int c = 0; c < n_steps; ++c) {
+      const uint32_t s = (uint32_t)rot(c);
+      const double2 b01 = ld_shared_f64x2(beta0 + s * 32u), b23 = ld_shared_f64x2(beta0 + s * 32u + 16u);
+      const float4 x = ld_step_f32<U>(xrow + s * 16u);
+      a0 = fma((double)x.x, b01.x, a0); a1 = fma((double)x.y, b01.y, a1);
+      a2 = fma((double)x.z, b23.x, a2); a3 = fma((double)x.w, b23.y, a3);
+    }
+    return (a0 + a1) + (a2 + a3);
+  } else {
+    // fp64 X: 2 elements per step, two steps per iteration -> 4 independent DFMA chains
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int c = 0;
+#pragma unroll 2
+    for (; c + 1 < n_steps; c += 2) {
+      const uint32_t s0 = (uint32_t)rot(c) * 16u, s1 = (uint32_t)rot(c + 1) * 16u;
+      const double2 b0 = ld_shared_f64x2(beta0 + s0), b1 = ld_shared_f64x2(beta0 + s1);
+      const double2 x0 = ld_step_f64<U>(xrow + s0), x1 = ld_step_f64<U>(xrow + s1);
+      a0 = fma(x0.x, b0.x, a0); a1 = fma(x0.y, b0.y, a1); a2 = fma(x1.x, b1.x, a2); a3 = fma(x1.y, b1.y, a3);
+    }
+    if (c < n_steps) {
+      const uint32_t s0 = (uint32_t)rot(c) * 16u;
+      const double2 b0 = ld_shared_f64x2(beta0 + s0);
+      const double2 x0 = ld_step_f64<U>(xrow + s0);
+      a0 = fma(x0.x, b0.x, a0); a1 = fma(x0.y, b0.y, a1);
+    }
+    return (a0 + a1) + (a2 + a3);
+  }
+}
+
+template <typename XT, int U, int EM>
 __global__ void __launch_bounds__(kNarrowThreads, 1)
 fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y, long long N, int p,
                   unsigned long long seed, const double* __restrict__ beta, const Ctl* __restrict__ ctl,
-                  double* __restrict__ partial, double* __restrict__ z_out, int S, int D, int RT, int L,
+                  double* __restrict__ partial, double* __restrict__ z_out, int S, int RT, int skew_shift,
                   long long n_tiles, long long row_off) {
   constexpr bool kF32 = sizeof(XT) == 4;
-  using Acc = typename std::conditional<kF32, float, double>::type;
+  constexpr bool kFloatAcc = kF32 && EM != 0;
+  constexpr int SE = 16 / (int)sizeof(XT);                 // elements per 16-byte step
   extern __shared__ __align__(128) unsigned char smem[];
   const size_t row_bytes = (size_t)p * sizeof(XT);
   const size_t stage_bytes = narrow_stage_bytes(RT, row_bytes);
-  const NarrowSmemLayout lay(S, RT, p, stage_bytes);
+  const NarrowSmemLayout lay(S, RT, stage_bytes);
   unsigned char* tiles = smem + lay.tiles;
-  double* eta_s = reinterpret_cast<double*>(smem + lay.eta);
   double* z64 = reinterpret_cast<double*>(smem + lay.z64);
   float* z32 = reinterpret_cast<float*>(smem + lay.z32);
   double* red = reinterpret_cast<double*>(smem + lay.red);
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + lay.bars);
   uint64_t* empty = full + S;
-  uint64_t* eta_full = empty + S;
-  uint64_t* z_full = eta_full + S;
+  uint64_t* z_full = empty + S;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const long long cta = blockIdx.x, grid = gridDim.x;
   const long long my_tiles = cta < n_tiles ? (n_tiles - cta + grid - 1) / grid : 0;
   const uint32_t sweep = (uint32_t)(ctl->sweep + 1ull);
+  const int BPT = RT / 32;
+  const int n_steps = (p + SE - 1) / SE;
 
   if (tid == 0) {
     for (int s = 0; s < S; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], kComputeWarpsAll);
-      mbar_init(&eta_full[s], kComputeWarpsAll);
-      mbar_init(&z_full[s], RT / 32);
+      mbar_init(&z_full[s], BPT);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -564,10 +702,16 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
     for (size_t o = (size_t)tid * 16; o < (size_t)S * stage_bytes; o += (size_t)kNarrowThreads * 16)
       *reinterpret_cast<uint4*>(tiles + o) = zero;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    // beta in the accumulation type of the eta phase, zero beyond p (the last step of a row reads up to SE - 1 past it)
+    for (int e = tid; e < n_steps * SE; e += kNarrowThreads) {
+      const double bv = e < p ? beta[e] : 0.0;
+      if constexpr (kFloatAcc) reinterpret_cast<float*>(smem + lay.beta)[e] = (float)bv;
+      else reinterpret_cast<double*>(smem + lay.beta)[e] = bv;
+    }
   }
   __syncthreads();
 
-  if (warp == kComputeWarpsAll + kNarrowSamplers) {
+  if (warp == kComputeWarpsAll + kNarrowZWarps) {
     // ===================== producer =====================
     if (lane == 0) {
       int st = 0;
@@ -592,27 +736,36 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
       }
     }
   } else if (warp >= kComputeWarpsAll) {
-    // ===================== sampler warps: batches of 32 rows (lane = row), dealt round-robin =====================
-    // Batch gb = tile * BPT + b goes to sampler warp gb mod ns, so the BPT = RT/32 batches of a tile are sampled in
-    // parallel by different warps; z_full[stage] counts BPT arrivals.  ns <= S * BPT: a warp then never waits on a
-    // stage whose previous use has not completed its eta phase (a parity wait two phases early would pass at once).
-    const int sw = warp - kComputeWarpsAll;
-    const int BPT = RT / 32;
-    const int ns = S * BPT < kNarrowSamplers ? S * BPT : kNarrowSamplers;
+    // ===================== z-warps: eta (thread per row) -> z, batches of 32 rows dealt round-robin =====================
+    // Batch gb = tile * BPT + b goes to z-warp gb mod ns.  ns <= S * BPT: a warp then never waits on a stage whose
+    // previous use it has not finished itself (a parity wait two phases early would pass at once).
+    const int zw = warp - kComputeWarpsAll;
+    const int ns = S * BPT < kNarrowZWarps ? S * BPT : kNarrowZWarps;
     const long long n_batches = my_tiles * BPT;
-    if (sw < ns) {
-      for (long long gb = sw; gb < n_batches; gb += ns) {
+    if (zw < ns) {
+      const uint32_t beta0 = smem_u32(smem + lay.beta);
+      const uint32_t tiles0 = smem_u32(tiles), rb = (uint32_t)row_bytes, sb = (uint32_t)stage_bytes;
+      const int delta = (U == 16) ? ((lane & 7) >> skew_shift) : 0;
+      auto load_y = [&](long long gb) -> int {
+        const long long n = gb / BPT;
+        const long long i = (cta + n * grid) * RT + (gb - n * BPT) * 32 + lane;
+        return (gb < n_batches && i < N) ? (int)y[i] : 1;
+      };
+      int y_next = load_y(zw);                       // y is prefetched one batch ahead (a lone 1-byte load under a saturated HBM)
+      for (long long gb = zw; gb < n_batches; gb += ns) {
         const long long n = gb / BPT;
         const int b = (int)(gb - n * BPT) * 32;
         const int st = (int)(n % S);
         const uint32_t ph = (uint32_t)((n / S) & 1);
         const long long i = (cta + n * grid) * RT + b + lane;
         const bool valid = i < N;
-        const int yi = valid ? (int)y[i] : 1;
+        const int yi = y_next;
+        y_next = load_y(gb + ns);
+        // the Philox uniform does not depend on eta: computed before waiting for the tile
         const double u = uniform_a(seed, (unsigned long long)(row_off + (valid ? i : 0)), sweep, TAG_Z);
         const double ystar = 2.0 * (double)yi - 1.0;
-        mbar_wait(&eta_full[st], ph);
-        const double eta = eta_s[st * RT + b + lane];
+        mbar_wait(&full[st], ph);
+        const double eta = narrow_row_dot<XT, U, EM>(tiles0 + (uint32_t)st * sb + (uint32_t)(b + lane) * rb, beta0, n_steps, delta);
         const double wpos = tnpos(ystar * eta, u);
         const double z = valid ? ystar * wpos : 0.0;
         z64[st * RT + b + lane] = z;
@@ -623,95 +776,63 @@ fused_pass_narrow(const XT* __restrict__ X, const unsigned char* __restrict__ y,
       }
     }
   } else {
-    // ===================== compute warps =====================
-    // eta mapping: lane group of L lanes per row
-    const int l = tid & (L - 1), rsub = tid / L, rows_per_pass = kComputeThreadsAll / L;
-    double bd[kF32 && EM != 0 ? 1 : EMAX];
-    float bf[kF32 && EM != 0 ? EMAX : 1];
-#pragma unroll
-    for (int e = 0; e < EMAX; ++e) {
-      const int j = l + e * L;
-      const double bv = (j < p) ? beta[j] : 0.0;
-      if constexpr (kF32 && EM != 0) bf[e] = (float)bv; else bd[e] = bv;
-    }
-    // xz mapping: thread t -> column t mod p, row group t div p
-    const int NG = kComputeThreadsAll / p > 0 ? kComputeThreadsAll / p : 1;   // p <= 512 here
+    // ===================== x*z warps =====================
+    // thread t -> column t mod p, row group t div p
+    const int NG = kComputeThreadsAll / p > 0 ? kComputeThreadsAll / p : 1;   // p <= 511 here
     const int xg = tid / p, xj = tid - xg * p;
     const bool xz_on = xg < NG;
     const int RPG = ((RT + NG - 1) / NG + 3) / 4 * 4;                      // rows of a tile per row group, a multiple of 4
+    const int r_lo = xg * RPG, r_hi = (xg + 1) * RPG < RT ? (xg + 1) * RPG : RT;
     const uint32_t z32a = smem_u32(z32), z64a = smem_u32(z64);
     double acc64 = 0.0;
-    Acc acc = (Acc)0;
+    typename std::conditional<kF32, unsigned long long, double>::type acc = 0;   // fp32 X: a packed pair of fp32 chains
+    auto acc_value = [&]() -> double {
+      if constexpr (kF32) { float a, b; f2_unpack(acc, a, b); return (double)a + (double)b; }
+      else return acc;
+    };
     const uint32_t rb = (uint32_t)row_bytes, sb = (uint32_t)stage_bytes;
-    const uint32_t tiles0 = smem_u32(tiles);
-    const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty), etaf0 = smem_u32(eta_full), zf0 = smem_u32(z_full);
-    uint32_t st_e = 0, st_g = 0, ph_e = 0, ph_g = 0;
+    const uint32_t xcol0 = smem_u32(tiles) + (uint32_t)xj * (uint32_t)sizeof(XT) + (uint32_t)r_lo * rb;
+    const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty), zf0 = smem_u32(z_full);
+    uint32_t st = 0, ph = 0;
     int rows_since_flush = 0;
-    const int n_my = (int)my_tiles, total_it = n_my + D;
-    for (int it = 0; it < total_it; ++it) {
-      if (it < n_my) {
-        mbar_wait_a(full0 + 8u * st_e, ph_e);
-        const uint32_t tile = tiles0 + st_e * sb;
-        for (int r = rsub; r < RT; r += rows_per_pass) {
-          const uint32_t xa = tile + (uint32_t)r * rb + (uint32_t)l * (uint32_t)sizeof(XT);
-          double s;
-          if constexpr (kF32 && EM != 0) {
-            float c = 0.f;
-#pragma unroll
-            for (int e = 0; e < EMAX; ++e) c = fmaf(ld_shared_f32(xa + (uint32_t)(e * L) * 4u), bf[e], c);   // past p: beta = 0
-#pragma unroll
-            for (int off = 16; off >= 1; off >>= 1)
-              if (off < L) c += __shfl_xor_sync(0xffffffffu, c, off);       // L is uniform: no divergence
-            s = (double)c;
-          } else {
-            s = 0.0;
-#pragma unroll
-            for (int e = 0; e < EMAX; ++e) s = fma((double)ld_shared_x<XT>(xa + (uint32_t)(e * L) * (uint32_t)sizeof(XT)), bd[e], s);
-#pragma unroll
-            for (int off = 16; off >= 1; off >>= 1)
-              if (off < L) s += __shfl_xor_sync(0xffffffffu, s, off);
-          }
-          if (l == 0) eta_s[st_e * RT + r] = s;
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive_a(etaf0 + 8u * st_e);
-        if (++st_e == (uint32_t)S) { st_e = 0; ph_e ^= 1u; }
-      }
-      if (it >= D) {
-        mbar_wait_a(zf0 + 8u * st_g, ph_g);
-        if (xz_on) {
-          // rows [xg RPG, (xg+1) RPG) of the tile, four at a time (z as one 16-byte / two 16-byte loads)
-          const uint32_t xa = tiles0 + st_g * sb + (uint32_t)xj * (uint32_t)sizeof(XT);
-          const int r_hi = (xg + 1) * RPG < RT ? (xg + 1) * RPG : RT;
-          if constexpr (kF32) {
-            const uint32_t za = z32a + (uint32_t)(st_g * RT) * 4u;
-            for (int r = xg * RPG; r < r_hi; r += 4) {
-              const float4 z4 = ld_shared_f32x4(za + (uint32_t)r * 4u);
-              const uint32_t x0 = xa + (uint32_t)r * rb;
-              const float a0 = ld_shared_f32(x0), a1 = ld_shared_f32(x0 + rb), a2 = ld_shared_f32(x0 + 2u * rb), a3 = ld_shared_f32(x0 + 3u * rb);
-              acc = fmaf(a0, z4.x, acc); acc = fmaf(a1, z4.y, acc); acc = fmaf(a2, z4.z, acc); acc = fmaf(a3, z4.w, acc);
-            }
-          } else {
-            const uint32_t za = z64a + (uint32_t)(st_g * RT) * 8u;
-            for (int r = xg * RPG; r < r_hi; r += 4) {
-              const double2 za01 = ld_shared_f64x2(za + (uint32_t)r * 8u), za23 = ld_shared_f64x2(za + (uint32_t)r * 8u + 16u);
-              const uint32_t x0 = xa + (uint32_t)r * rb;
-              const double a0 = ld_shared_f64(x0), a1 = ld_shared_f64(x0 + rb), a2 = ld_shared_f64(x0 + 2u * rb), a3 = ld_shared_f64(x0 + 3u * rb);
-              acc = fma(a0, za01.x, acc); acc = fma(a1, za01.y, acc); acc = fma(a2, za23.x, acc); acc = fma(a3, za23.y, acc);
-            }
-          }
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive_a(empty0 + 8u * st_g);
-        if (++st_g == (uint32_t)S) { st_g = 0; ph_g ^= 1u; }
+    const int n_my = (int)my_tiles;
+    for (int it = 0; it < n_my; ++it) {
+      mbar_wait_a(zf0 + 8u * st, ph);
+      mbar_wait_a(full0 + 8u * st, ph);          // complete long ago; orders this thread's reads after the bulk copy
+      if (xz_on && r_lo < r_hi) {
+        uint32_t x0 = xcol0 + st * sb;
         if constexpr (kF32) {
-          rows_since_flush += RPG;
-          if (rows_since_flush >= kFlushRows) { rows_since_flush = 0; acc64 += (double)acc; acc = 0.f; }
+          uint32_t za = z32a + (uint32_t)(st * RT + r_lo) * 4u;
+#pragma unroll 2
+          for (int r = r_lo; r < r_hi; r += 4) {
+            unsigned long long z01, z23;
+            ld_shared_b64x2(za, z01, z23);
+            const float a0 = ld_shared_f32(x0), a1 = ld_shared_f32(x0 + rb), a2 = ld_shared_f32(x0 + 2u * rb), a3 = ld_shared_f32(x0 + 3u * rb);
+            acc = f2_fma(f2_pack(a0, a1), z01, acc);      // even rows in the low half, odd rows in the high half
+            acc = f2_fma(f2_pack(a2, a3), z23, acc);
+            za += 16u; x0 += 4u * rb;
+          }
+        } else {
+          uint32_t za = z64a + (uint32_t)(st * RT + r_lo) * 8u;
+#pragma unroll 2
+          for (int r = r_lo; r < r_hi; r += 4) {
+            const double2 za01 = ld_shared_f64x2(za), za23 = ld_shared_f64x2(za + 16u);
+            const double a0 = ld_shared_f64(x0), a1 = ld_shared_f64(x0 + rb), a2 = ld_shared_f64(x0 + 2u * rb), a3 = ld_shared_f64(x0 + 3u * rb);
+            acc = fma(a0, za01.x, acc); acc = fma(a1, za01.y, acc); acc = fma(a2, za23.x, acc); acc = fma(a3, za23.y, acc);
+            za += 32u; x0 += 4u * rb;
+          }
         }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive_a(empty0 + 8u * st);
+      if (++st == (uint32_t)S) { st = 0; ph ^= 1u; }
+      if constexpr (kF32) {
+        rows_since_flush += RPG;
+        if (rows_since_flush >= kFlushRows) { rows_since_flush = 0; acc64 += acc_value(); acc = 0ull; }
       }
     }
-    // combine the NG row groups of every column in fixed order (named barrier over the 16 compute warps)
-    red[tid] = acc64 + (double)acc;
+    // combine the NG row groups of every column in fixed order (named barrier over the 16 x*z warps)
+    red[tid] = acc64 + acc_value();
     asm volatile("bar.sync 1, %0;" ::"n"(kComputeThreadsAll) : "memory");
     if (tid < p) {
       double s = 0.0;
@@ -844,28 +965,33 @@ static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* 
   const size_t elem = dtype == kF32 ? 4 : 8;
   const size_t row_bytes = (size_t)p * elem;
   // tiny problems (C1) are launch-bound: the generic kernel has no 224 KB ring to set up
-  if ((reinterpret_cast<uintptr_t>(X) & 15) != 0 || p > kComputeThreadsAll - 1 || (size_t)N * row_bytes < ((size_t)2 << 20)) return false;
-  int L = 1;
-  while (L < 32 && (p + L - 1) / L > 4) L <<= 1;
-  const int E = (p + L - 1) / L;
-  if (E > 16) return false;
-  int RT = (int)(56000 / row_bytes) / 32 * 32;      // ~50 KB stages (4 fit): the per-tile overhead is what limits narrow rows
+  if ((reinterpret_cast<uintptr_t>(X) & 15) != 0 || p > kNarrowMaxP || (size_t)N * row_bytes < ((size_t)2 << 20)) return false;
+  // U: unit of the thread-per-row dot product; skew for rows that are an even number of 16-byte units (see the kernel)
+  int U = 16;
+  while (row_bytes % (size_t)U) U >>= 1;
+  int shift = 3;
+  if (U == 16) {
+    const size_t q = row_bytes / 16;
+    int g = 1;
+    while (g < 8 && q % (size_t)(2 * g) == 0) g <<= 1;       // gcd(q, 8)
+    shift = g == 1 ? 3 : g == 2 ? 2 : g == 4 ? 1 : 0;
+  }
+  // ~36 KB stages, five or six in the ring (measured at the R1 shape, 564-byte rows: 64 rows x 5 stages 6.0 TB/s; 32 x 12 and
+  // 96 x 3 5.4-5.6 TB/s; 64 x 4 5.3 TB/s)
+  int RT = ((int)(36000 / row_bytes) + 16) / 32 * 32;
   RT = RT < 32 ? 32 : RT > 256 ? 256 : RT;
   if (opt.narrow_rt > 0) RT = opt.narrow_rt / 32 * 32;
+  if (RT < 32) RT = 32;
   const size_t stage_bytes = narrow_stage_bytes(RT, row_bytes);
   const size_t budget = 227 * 1024;
   int S = opt_or(opt.fused_stages, 0);
   if (S <= 0) {
-    S = 8;
-    while (S > 2 && NarrowSmemLayout(S, RT, p, stage_bytes).total > budget) --S;
+    S = 12;
+    while (S > 2 && NarrowSmemLayout(S, RT, stage_bytes).total > budget) --S;
   }
-  if (S < 3 || NarrowSmemLayout(S, RT, p, stage_bytes).total > budget) return false;
-  int D = opt_or(opt.fused_lag, 0);
-  if (D <= 0) D = (S - 1) / 2 > 2 ? (S - 1) / 2 : 2;
-  if (D > S - 2) D = S - 2;
-  if (D < 1) D = 1;
+  if (S < 3 || NarrowSmemLayout(S, RT, stage_bytes).total > budget) return false;
   pl->variant = 2;
-  pl->rows_per_tile = RT; pl->chunks = E <= 4 ? 4 : E <= 6 ? 6 : E <= 8 ? 8 : E <= 12 ? 12 : 16; pl->width = L; pl->stages = S; pl->lag = D;
+  pl->rows_per_tile = RT; pl->chunks = U; pl->width = shift; pl->stages = S; pl->lag = 0;
   pl->groups = 1;
   int em = dtype == kF32 ? opt_or(opt.fused_eta, 2) : 0;
   pl->eta_mode = (em == 0) ? 0 : 2;
@@ -873,20 +999,20 @@ static bool narrow_plan(int dtype, long long N, int p, int num_sms, const void* 
   int grid = opt.fused_grid > 0 ? opt.fused_grid : num_sms;
   if ((long long)grid > pl->n_tiles) grid = (int)pl->n_tiles;
   pl->grid = grid; pl->block = kNarrowThreads;
-  pl->smem = NarrowSmemLayout(S, RT, p, stage_bytes).total;
+  pl->smem = NarrowSmemLayout(S, RT, stage_bytes).total;
   return true;
 }
 
-template <typename XT, int EMAX, int EM>
+template <typename XT, int U, int EM>
 static cudaError_t launch_narrow(const FusedPlan& pl, const void* X, const unsigned char* y, long long N, int p,
                                  unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                                  double* z_out, cudaStream_t st) {
-  auto kern = fused_pass_narrow<XT, EMAX, EM>;
+  auto kern = fused_pass_narrow<XT, U, EM>;
   // prepare-only call (hsp_create, once per chain, outside stream capture): the attribute is per DEVICE, so it is
   // set for the current device every time a chain is created, not once per process
   if (N < 0) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
   kern<<<pl.grid, pl.block, pl.smem, st>>>(static_cast<const XT*>(X), y, N, p, seed, beta, ctl, partial, z_out,
-                                          pl.stages, pl.lag, pl.rows_per_tile, pl.width, pl.n_tiles, pl.row_offset);
+                                          pl.stages, pl.rows_per_tile, pl.width, pl.n_tiles, pl.row_offset);
   return cudaGetLastError();
 }
 
@@ -895,17 +1021,15 @@ static cudaError_t dispatch_narrow(const FusedPlan& pl, const void* X, const uns
                                    unsigned long long seed, const double* beta, const Ctl* ctl, double* partial,
                                    double* z_out, cudaStream_t st) {
 #define HSP_NARROW_ARGS pl, X, y, N, p, seed, beta, ctl, partial, z_out, st
-#define HSP_NARROW_CASE(E_)                                                                   \
-  if (pl.chunks == E_) {                                                                      \
+#define HSP_NARROW_CASE(U_)                                                                   \
+  if (pl.chunks == U_) {                                                                      \
     if constexpr (sizeof(XT) == 4) {                                                          \
-      if (pl.eta_mode == 2) return launch_narrow<XT, E_, 2>(HSP_NARROW_ARGS);                 \
+      if (pl.eta_mode == 2) return launch_narrow<XT, U_, 2>(HSP_NARROW_ARGS);                 \
     }                                                                                         \
-    return launch_narrow<XT, E_, 0>(HSP_NARROW_ARGS);                                         \
+    return launch_narrow<XT, U_, 0>(HSP_NARROW_ARGS);                                         \
   }
-  HSP_NARROW_CASE(4)
-  HSP_NARROW_CASE(6)
+  if constexpr (sizeof(XT) == 4) { HSP_NARROW_CASE(4) }
   HSP_NARROW_CASE(8)
-  HSP_NARROW_CASE(12)
   HSP_NARROW_CASE(16)
 #undef HSP_NARROW_CASE
 #undef HSP_NARROW_ARGS

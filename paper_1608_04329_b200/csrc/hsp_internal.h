@@ -40,7 +40,7 @@ struct Options {
 inline int opt_or(int v, int dflt) { return v >= 0 ? v : dflt; }
 
 struct FusedPlan {
-  int variant;        // 0 = generic, 1 = tma (wide rows), 2 = tma-narrow (width = L lanes per row, chunks = EMAX)
+  int variant;        // 0 = generic, 1 = tma (wide rows), 2 = tma-narrow (chunks = U bytes per load of the row dot product, width = skew shift)
   int grid, block;
   size_t smem;
   int rows_per_tile;  // R

@@ -220,28 +220,45 @@ def test_tensor_core_gram_matches_fp64_definition(name, n, p, hsp_options):
     run_parity(hsp_synth.make(name, "cuda", n_rows=n, p=p), 4, gram=Go)
 
 
-# ---- fused_pass_narrow: every instantiation the default dispatch can reach (fused_pass.cu narrow_plan: EMAX in
-# {4, 6, 8, 12, 16} elements per lane, fp32 chains and exact fp64), whole sweeps against the oracle
+# ---- fused_pass_narrow: every instantiation the default dispatch can reach (fused_pass.cu narrow_plan): the row is
+# read in units of U = 4, 8 or 16 bytes (the largest power of two dividing the row), and rows of an even number q of
+# 16-byte units are read with a per-lane start offset (skew shift 2, 1, 0 for gcd(q, 8) = 2, 4, 8); fp32 chains and exact
+# fp64.  Whole sweeps against the oracle.
 NARROW_CASES = [
-    # config (dtype), rows, p, elements per lane E = ceil(p / 32)
-    ("C3", 12001, 200, 7),    # fp32, EMAX 8
-    ("C3", 9001, 250, 8),     # fp32, EMAX 8
-    ("C3", 6007, 400, 13),    # fp32, EMAX 16
-    ("C3", 5003, 511, 16),    # fp32, EMAX 16, the widest row the narrow kernel takes
-    ("C3", 9001, 180, 6),     # fp32, EMAX 6
-    ("C3", 6007, 300, 10),    # fp32, EMAX 12
-    ("C3", 20011, 100, 4),    # fp32, EMAX 4
-    ("C2", 6007, 150, 5),     # fp64, EMAX 6
-    ("C2", 4001, 250, 8),     # fp64, EMAX 8
-    ("C2", 5003, 190, 6),     # fp64, EMAX 6
-    ("C2", 4001, 280, 9),     # fp64, EMAX 12
+    # config (dtype), rows, p, U, skew shift (3 = none)
+    ("C3", 9001, 141, 4, 3),      # fp32, 564-byte rows: the shape of the paper's real-data run
+    ("C3", 5003, 511, 4, 3),      # fp32, the widest row the narrow kernel takes
+    ("C3", 9001, 250, 8, 3),      # fp32, 1000-byte rows
+    ("C3", 20011, 100, 16, 3),    # fp32, q = 25
+    ("C3", 9001, 180, 16, 3),     # fp32, q = 45
+    ("C3", 12001, 200, 16, 2),    # fp32, q = 50: gcd 2
+    ("C3", 6007, 400, 16, 1),     # fp32, q = 100: gcd 4
+    ("C3", 24001, 96, 16, 0),     # fp32, q = 24: gcd 8
+    ("C3", 32003, 17, 4, 3),      # fp32, very narrow rows (30 row groups in the x*z phase)
+    ("C2", 6007, 150, 16, 3),     # fp64, q = 75
+    ("C2", 5003, 101, 8, 3),      # fp64, 808-byte rows
+    ("C2", 5003, 190, 16, 3),     # fp64, q = 95
+    ("C2", 4001, 250, 16, 3),     # fp64, q = 125
+    ("C2", 6007, 100, 16, 2),     # fp64, q = 50 (C2's own row width)
+    ("C2", 5003, 252, 16, 2),     # fp64, q = 126: gcd 2, the widest fp64 rows just below the wide kernel
+    ("C2", 8009, 64, 16, 0),      # fp64, q = 32: gcd 8
 ]
 
 
-@pytest.mark.parametrize("name,n_rows,p,E", NARROW_CASES)
-def test_narrow_kernel_every_instantiation_whole_sweeps(name, n_rows, p, E):
+def _check_narrow_case(wl, U, shift):
+    rb = wl.p * wl.X.element_size()
+    assert rb % U == 0 and (U == 16 or rb % (2 * U) != 0)
+    if U == 16:
+        q, g = rb // 16, 1
+        while g < 8 and q % (2 * g) == 0:
+            g *= 2
+        assert shift == {1: 3, 2: 2, 4: 1, 8: 0}[g]
+
+
+@pytest.mark.parametrize("name,n_rows,p,U,shift", NARROW_CASES)
+def test_narrow_kernel_every_instantiation_whole_sweeps(name, n_rows, p, U, shift):
     wl = hsp_synth.make(name, "cuda", n_rows=n_rows, p=p)
-    assert (p + 31) // 32 == E
+    _check_narrow_case(wl, U, shift)
     X64 = wl.X.double()
     probe = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
     assert probe.fused_variant() == "tma-narrow"
@@ -250,9 +267,14 @@ def test_narrow_kernel_every_instantiation_whole_sweeps(name, n_rows, p, E):
     assert w["z"] < (2e-6 if wl.X.dtype == torch.float32 else 1e-9)
 
 
-@pytest.mark.parametrize("name,n_rows,p,E", NARROW_CASES)
-def test_narrow_kernel_fused_pass_only(name, n_rows, p, E):
-    """a1-a3 + b alone at a planted beta (scales and beta frozen): z and X^T z against the oracle."""
+@pytest.mark.parametrize("eta_mode", [2, 0])
+@pytest.mark.parametrize("name,n_rows,p,U,shift", NARROW_CASES)
+def test_narrow_kernel_fused_pass_only(name, n_rows, p, U, shift, eta_mode, hsp_options):
+    """a1-a3 + b alone at a planted beta (scales and beta frozen): z and X^T z against the oracle, in both arithmetic
+    modes of the eta phase for fp32 X (fp32 chains / exact fp64)."""
+    if name == "C2" and eta_mode == 0:
+        pytest.skip("fp64 X has one eta mode")
+    hsp_options("fused_eta", eta_mode)
     wl = hsp_synth.make(name, "cuda", n_rows=n_rows + 13, p=p)
     Xh, yh = wl.host()
     beta = wl.beta_true * 0.6
@@ -267,7 +289,7 @@ def test_narrow_kernel_fused_pass_only(name, n_rows, p, E):
     zg, sg = g.get_latent(); zo, so = o.get_latent()
     assert np.array_equal(sg, so)
     ez, eg = mixed_err(zg, zo), mixed_err(g.get_xtz(), o.get_xtz())
-    print(name, n_rows, p, "E", E, "narrow fused pass only: z", ez, "xtz", eg)
+    print(name, n_rows, p, "U", U, "shift", shift, "eta mode", eta_mode, "narrow fused pass only: z", ez, "xtz", eg)
     f32 = wl.X.dtype == torch.float32
-    assert ez < (2e-6 if f32 else 1e-11) and eg < (1e-5 if f32 else 1e-11)
+    assert ez < ((2e-6 if eta_mode else 1e-9) if f32 else 1e-11) and eg < (1e-5 if f32 else 1e-11)
     g.close()
