@@ -18,6 +18,7 @@
 #include <algorithm>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <functional>
 #include <queue>
 #include <vector>
@@ -29,7 +30,7 @@ namespace {
 
 struct Cost { double mac = 3.3, hop = 2.0, potrf = 8.0, trinv = 3.0, store = 0.9, loadp = 0.5, cmac = 2.6; };   // us, from the chol_trace option at p = 1000 (cmac: a product of the chain CTA, operands in shared memory)
 
-struct Step { double cost; int dep[2]; };                 // deps are task ids (-1 = none)
+struct Step { double cost; int dep[2]; bool local = false; };   // deps are task ids (-1 = none); local: dep[0] ran on the same CTA (no flag hop)
 struct Node {
   CholTask t;
   std::vector<Step> steps;
@@ -65,16 +66,16 @@ Graph build_graph(int nt, int sb, const Cost& c, bool chain) {
         g.n[pd].steps.push_back(Step{c.store, {-1, -1}});
       }
       const int po = add(CholTask{2, j, j, 0, 0, -1, -1, 0});
-      g.n[po].steps.push_back(Step{c.potrf + c.trinv + c.store, {prev, -1}});
+      g.n[po].steps.push_back(Step{c.potrf + c.trinv + c.store, {prev, -1}, true});
       g.chain.push_back(po); prev = po;
       idL[(size_t)j * nt + j] = po;
       if (j + 1 < nt) {
         const int tr = add(CholTask{3, j + 1, j, 0, 0, slot_s, -1, 0});
-        g.n[tr].steps.push_back(Step{c.loadp + c.cmac + c.store, {po, ps}});
+        g.n[tr].steps.push_back(Step{c.loadp + c.cmac + c.store, {po, ps}, true});
         g.chain.push_back(tr);
         idL[(size_t)(j + 1) * nt + j] = tr;
         const int sy = add(CholTask{4, j + 1, j, 0, 0, slot_d, -1, 0});
-        g.n[sy].steps.push_back(Step{c.loadp + c.cmac, {tr, pd}});
+        g.n[sy].steps.push_back(Step{c.loadp + c.cmac, {tr, pd}, true});
         g.chain.push_back(sy); prev = sy;
       }
       for (int i = j + 2; i < nt; ++i) {
@@ -158,7 +159,7 @@ inline void run_task(const Node& nd, double start, const std::vector<double>& fi
   double cur = start, id = 0.0;
   for (const Step& s : nd.steps) {
     double r = 0.0;
-    for (int d : s.dep) if (d >= 0) r = std::max(r, finish[d] + hop);
+    for (int q = 0; q < 2; ++q) if (s.dep[q] >= 0) r = std::max(r, finish[s.dep[q]] + (q == 0 && s.local ? 0.0 : hop));
     if (r > cur) { id += r - cur; cur = r; }
     cur += s.cost;
   }
@@ -169,15 +170,17 @@ inline void run_task(const Node& nd, double start, const std::vector<double>& fi
 
 CholSchedule chol_build_schedule(int nt, int sb, int K) {
   const Cost c;
-  Graph g = build_graph(nt, sb, c);
+  const bool big = nt > 96;                              // the greedy search is quadratic in the task count
+  const bool chain = K >= 2 && nt >= 2 && !big;          // list 0 = the chain CTA, lists 1.. = everything else
+  Graph g = build_graph(nt, sb, c, chain);
   const int T = (int)g.n.size();
   CholSchedule out;
   out.K = K; out.n_slots = g.n_slots;
   std::vector<std::vector<int>> lists(K);
   std::vector<double> finish(T, 0.0);
-  if (nt > 96 || K == 1) {
-    // very large problems: the greedy search is quadratic in the task count; deal the tasks round-robin in
-    // id order (a valid global order: every producer has a smaller id or is an L tile of an earlier column)
+  if (big || K == 1) {
+    // deal the tasks round-robin in id order (a valid global order: every producer has a smaller id or is an
+    // L tile of an earlier column)
     std::vector<int> order(T);
     for (int a = 0; a < T; ++a) order[a] = a;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
@@ -195,14 +198,39 @@ CholSchedule chol_build_schedule(int nt, int sb, int K) {
       lists[cta].push_back(a);
     }
   } else {
-    std::vector<char> in_cand(T, 0), placed_v(T, 0);
+    std::vector<char> in_cand(T, 0), placed_v(T, 0), is_chain(T, 0);
+    for (int a : g.chain) is_chain[a] = 1;
     std::vector<int> cand;
-    for (int a = 0; a < T; ++a) if (g.n[a].prod.empty()) { cand.push_back(a); in_cand[a] = 1; }
+    int placed = 0;
+    size_t chain_pos = 0;
+    double chain_free = 0.0;
+    auto ready = [&](int a) {
+      for (int d : g.n[a].prod) if (!placed_v[d]) return false;
+      return true;
+    };
+    auto release = [&](int a) {                            // consumers of a placed task become candidates
+      for (auto& cs : g.n[a].cons)
+        if (!in_cand[cs.first] && !is_chain[cs.first] && ready(cs.first)) { cand.push_back(cs.first); in_cand[cs.first] = 1; }
+    };
+    // the chain CTA takes its next task as soon as all its producers are placed (placement order = the global order)
+    auto advance_chain = [&]() {
+      while (chain_pos < g.chain.size() && ready(g.chain[chain_pos])) {
+        const int a = g.chain[chain_pos++];
+        double e, idle;
+        run_task(g.n[a], chain_free, finish, c.hop, &e, &idle);
+        finish[a] = e; chain_free = e; placed_v[a] = 1; ++placed;
+        lists[0].push_back(a);
+        release(a);
+      }
+    };
+    for (int a = 0; a < T; ++a) if (!is_chain[a] && g.n[a].prod.empty()) { cand.push_back(a); in_cand[a] = 1; }
     using Ev = std::pair<double, int>;
     std::priority_queue<Ev, std::vector<Ev>, std::greater<Ev>> free_q;
-    for (int k = 0; k < K; ++k) free_q.push({0.0, k});
+    for (int k = chain ? 1 : 0; k < K; ++k) free_q.push({0.0, k});
     const double idle_ok = 1.0;
-    for (int placed = 0; placed < T; ++placed) {
+    advance_chain();
+    while (placed < T) {
+      if (cand.empty()) { fprintf(stderr, "chol_build_schedule: no candidate (nt=%d K=%d)\n", nt, K); abort(); }
       const Ev ev = free_q.top(); free_q.pop();
       int best = -1; double best_end = 0.0, best_rank = -1.0;
       int fb = -1; double fb_end = 0.0, fb_idle = 1e300, fb_rank = -1.0;
@@ -218,16 +246,11 @@ CholSchedule chol_build_schedule(int nt, int sb, int K) {
       const int a = best >= 0 ? best : fb;
       const double e = best >= 0 ? best_end : fb_end;
       cand.erase(std::find(cand.begin(), cand.end(), a));
-      finish[a] = e; placed_v[a] = 1;
+      finish[a] = e; placed_v[a] = 1; ++placed;
       lists[ev.second].push_back(a);
       free_q.push({e, ev.second});
-      for (auto& cs : g.n[a].cons)
-        if (!in_cand[cs.first]) {
-          // a consumer becomes a candidate once all its producers are placed
-          bool all = true;
-          for (int d : g.n[cs.first].prod) if (!placed_v[d]) { all = false; break; }
-          if (all) { cand.push_back(cs.first); in_cand[cs.first] = 1; }
-        }
+      release(a);
+      advance_chain();
     }
   }
   out.list_off.assign(K + 1, 0);
