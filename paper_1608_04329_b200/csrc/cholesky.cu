@@ -70,8 +70,17 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
   return t;
 }
-__device__ __forceinline__ void wait_flag(const int* f) {
-  while (ld_acquire(f) == 0) __nanosleep(20);
+// Flag protocol (the pattern of a CTA-wide semaphore): the producer CTA finishes its global stores, __syncthreads(), and
+// ONE thread publishes with st.release.gpu; the consumer polls with ld.acquire.gpu from ONE thread (or the lanes of ONE
+// warp, for many flags at once) and then __syncthreads().  An acquire load costs an L1 invalidation (SASS CCTL.IVALL);
+// polled by every warp before every k-tile it was 20 % of the kernel's stall samples at p = 4000.
+__device__ __forceinline__ void wait_flag_cta(const int* f, int tid) {
+  if (tid == 0)
+    while (ld_acquire(f) == 0) __nanosleep(20);
+  __syncthreads();
+}
+__device__ __forceinline__ void cp_async16_s(uint32_t dst_smem, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
 }
 
 // D(8x8) += A(8x4) B(4x8) on the FP64 tensor pipe.  Fragments (PTX ISA, m8n8k4 .f64): with g = lane / 4,
@@ -292,9 +301,13 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
   double* S = pool + kPoolDoubles;                   // 64 x TLD
   double* X = S + CT * TLD;                          // 64 x TLD
   double* rdiag = X + CT * TLD;                      // 64
+  __shared__ int s_ready[2];                         // result of the last two flag scans (double-buffered)
   const int P = nt * CT;
   const int tid = threadIdx.x;
   const Frag f(tid);
+  const uint32_t pool_s = (uint32_t)__cvta_generic_to_shared(pool);
+  const uint32_t x_s = pool_s + (uint32_t)((kPoolDoubles + CT * TLD) * sizeof(double));
+  int scan_par = 0;
   int* fL = flags;
   int* fB = flags + (size_t)nt * nt;
   int* fP = fB + (size_t)nt * nt;
@@ -318,7 +331,7 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
         }
   };
   auto load_slot = [&](int slot, double (&a)[4][2][2]) {
-    wait_flag(&fP[slot]);
+    wait_flag_cta(&fP[slot], tid);
     const double2* src = reinterpret_cast<const double2*>(ws + (size_t)slot * CT * CT);
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
@@ -350,7 +363,6 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       if (Lt != nullptr)   // L^T, used by the block back-substitution when only a block-diagonal inverse is built
         *reinterpret_cast<double2*>(Lt + g) = make_double2(c >= r ? S[c * TLD + r] : 0.0, c + 1 >= r ? S[(c + 1) * TLD + r] : 0.0);
     }
-    __threadfence();
     __syncthreads();
     if (tid == 0) st_release(&fL[(size_t)j_ * nt + j_], 1);
   };
@@ -391,7 +403,6 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
           }
         __syncthreads();                              // the product has been read from S by every warp
         acc_to_smem(out, S);
-        __threadfence();
         __syncthreads();
         if (tid == 0) st_release(&fL[(size_t)(j + 1) * nt + j], 1);
       } else {
@@ -426,22 +437,46 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
     }
 
     const int nchunks = (kend - kbeg) * (CT / KC);
+    // operand flags of k-tile k: L(ra,k) and L(rb,k) (L tasks), L(ra,k) and Wt(rb,k) (inverse tiles)
+    auto k_ready = [&](int k) -> bool {
+      bool ok = ld_acquire(&fL[(size_t)ra * nt + k]) != 0;
+      if (isL) { if (rb != ra) ok = (ld_acquire(&fL[(size_t)rb * nt + k]) != 0) && ok; }
+      else ok = (ld_acquire(k == rb ? &fL[(size_t)rb * nt + rb] : &fB[(size_t)rb * nt + k]) != 0) && ok;
+      return ok;
+    };
+    // warp 0 looks at the flags of up to 32 k-tiles from k0 on (a lane each), spins until k0 itself is ready and
+    // publishes the first k that is NOT known to be ready; every thread returns it
+    auto scan = [&](int k0) -> int {
+      scan_par ^= 1;
+      if (tid < 32) {
+        const int k = k0 + tid;
+        int n;
+        for (;;) {
+          const bool ok = k < kend ? k_ready(k) : false;
+          const unsigned m = __ballot_sync(0xffffffffu, ok);
+          n = __ffs(~m) - 1;
+          if (n < 0) n = 32;
+          if (n > 0) break;
+          __nanosleep(20);
+        }
+        if (tid == 0) s_ready[scan_par] = k0 + n;
+      }
+      __syncthreads();
+      return s_ready[scan_par];
+    };
+    int k_known = kbeg;                              // k-tiles below this are known to be ready
+    const int ld_row = tid >> 4, ld_pc = (tid & 15) * 2;
     auto issue = [&](int c) {
       const int k = kbeg + c / (CT / KC), kc = c % (CT / KC);
-      if (kc == 0) {                                 // first chunk of a k tile: its producers must be done
-        wait_flag(&fL[(size_t)ra * nt + k]);
-        if (isL) { if (rb != ra) wait_flag(&fL[(size_t)rb * nt + k]); }
-        else wait_flag(k == rb ? &fL[(size_t)rb * nt + rb] : &fB[(size_t)rb * nt + k]);
-      }
-      double* sa = pool + (size_t)(c % NST) * kStageDoubles;
-      double* sb = sa + CT * CLD;
-      const double* ga = MA + (size_t)ra * CT * P + (size_t)k * CT + kc * KC;
-      const double* gb = MB + (size_t)rb * CT * P + (size_t)k * CT + kc * KC;
+      if (kc == 0 && k >= k_known) k_known = scan(k);   // first chunk of a k tile: its producers must be done
+      const uint32_t sa = pool_s + (uint32_t)((c % NST) * kStageDoubles * sizeof(double)) + (uint32_t)((ld_row * CLD + ld_pc) * sizeof(double));
+      const uint32_t sb = sa + (uint32_t)(CT * CLD * sizeof(double));
+      const double* ga = MA + (size_t)ra * CT * P + (size_t)k * CT + kc * KC + (size_t)ld_row * P + ld_pc;
+      const double* gb = MB + (size_t)rb * CT * P + (size_t)k * CT + kc * KC + (size_t)ld_row * P + ld_pc;
 #pragma unroll
-      for (int q = tid; q < CT * (KC / 2); q += kCholThreads) {
-        const int row = q / (KC / 2), pc = q % (KC / 2);
-        cp_async16(sa + row * CLD + pc * 2, ga + (size_t)row * P + pc * 2);
-        cp_async16(sb + row * CLD + pc * 2, gb + (size_t)row * P + pc * 2);
+      for (int it = 0; it < CT / 16; ++it) {
+        cp_async16_s(sa + (uint32_t)(it * 16 * CLD * sizeof(double)), ga + (size_t)it * 16 * P);
+        cp_async16_s(sb + (uint32_t)(it * 16 * CLD * sizeof(double)), gb + (size_t)it * 16 * P);
       }
     };
     __syncthreads();                                 // the pool, S and X are free (previous task is over)
@@ -465,7 +500,6 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       double2* dst = reinterpret_cast<double2*>(ws + (size_t)tk.slot_out * CT * CT);
 #pragma unroll
       for (int q = 0; q < 8; ++q) __stcg(dst + q * kCholThreads + tid, make_double2(acc[q >> 1][q & 1][0], acc[q >> 1][q & 1][1]));
-      __threadfence();
       __syncthreads();
       if (tid == 0) st_release(&fP[tk.slot_out], 1);
     } else if (isL && i == j) {
@@ -475,11 +509,12 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       diag_finish(j);
     } else {
       // ---- off-diagonal: multiply by W_jj (from global; written by the diagonal task of column j)
-      wait_flag(&fL[(size_t)j * nt + j]);
+      wait_flag_cta(&fL[(size_t)j * nt + j], tid);
       const double* wjj = W + (size_t)j * CT * P + (size_t)j * CT;
-      for (int q = tid; q < CT * (CT / 2); q += kCholThreads) {
-        const int row = q / (CT / 2), pc = q % (CT / 2);
-        cp_async16(X + row * TLD + pc * 2, wjj + (size_t)row * P + pc * 2);
+#pragma unroll
+      for (int it = 0; it < CT / 8; ++it) {
+        const int row = (tid >> 5) + it * 8, pc = (tid & 31) * 2;
+        cp_async16_s(x_s + (uint32_t)((row * TLD + pc) * sizeof(double)), wjj + (size_t)row * P + pc);
       }
       cp_async_commit();
       double out[4][2][2];
@@ -506,7 +541,6 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
             *reinterpret_cast<double2*>(L + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
             if (Lt != nullptr) { Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1]; }
           }
-        __threadfence();
         __syncthreads();
         if (tid == 0) st_release(&fL[(size_t)i * nt + j], 1);
       } else {
@@ -529,7 +563,6 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
             Wt[(size_t)c * P + r] = out[mb][nb][0];
             Wt[(size_t)(c + 1) * P + r] = out[mb][nb][1];
           }
-        __threadfence();
         __syncthreads();
         if (tid == 0) st_release(&fB[(size_t)i * nt + j], 1);
       }
@@ -544,6 +577,7 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
 // Both kernels are launched with programmatic stream serialisation: the first pass over the row of W / Wt
 // (ready since the Cholesky branch joined) and the normal variate are issued BEFORE griddepcontrol.wait,
 // i.e. while the preceding kernel (reduce / first product) is still running.
+constexpr double kPassSatSms = 112.0;              // SMs at which the fused pass saturates HBM (measured: 116 -> 7.1 TB/s)
 constexpr int kGemvWarps = 4;
 constexpr int kGemvPass = 1024;                      // columns per pass: 32 lanes x 16 double2
 
@@ -758,6 +792,20 @@ cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_e
           const double t = std::max(fused_us * num_sms / (num_sms - k), 1.25 * s.makespan_us);
           if (t < best_t) { best_t = t; best = std::move(s); found = true; }
         }
+      // A large branch (p >= ~2000) that is longer than the pass: split the SMs so that both finish together.  The pass
+      // streams X at full HBM bandwidth on ~kPassSatSms SMs and slows down in proportion below that; the branch is
+      // bound by its work on few SMs and by the chain of diagonal tiles on many.  A split that does not beat running
+      // the two one after the other on every SM by 10 % is not taken.
+      if (!found && nt > 20) {
+        double split_t = 0.9 * best_t;
+        for (int k : {64, 80, 96, 104, 112, 120, 128}) {
+          if (k > tile_tasks || k > num_sms - 16) break;
+          CholSchedule s = chol_build_schedule(nt, sb, k);
+          const double pass_us = fused_us * std::max(1.0, kPassSatSms / (double)(num_sms - k));
+          const double t = std::max(pass_us, 1.15 * s.makespan_us);   // 1.15: tile loads compete with the X stream
+          if (t < split_t) { split_t = t; best = std::move(s); found = true; }
+        }
+      }
       if (!found) best = std::move(serial);
     }
     pl->overlap = found;
