@@ -200,6 +200,13 @@ int hsp_dbg_cheng(double alpha, unsigned long long seed, unsigned sweep0, double
  * without the trace).  Returns the number of tasks (rows may be NULL to query it), or a negative status.
  * Synchronises.                                                                                     */
 long long hsp_dbg_chol_trace(const hsp_state* s, long long* rows, long long capacity);
+/* Host-only (no device needed): the static schedule the library would build for nt tile rows (64 x 64 tiles), inverse
+ * super-blocks of sb tiles and K CTAs.  rows: HOST, capacity x 8 int per task, the K per-CTA lists concatenated:
+ * {cta, type, i, j, kbeg, kend, slot_in, slot_out}; task types: 0 tile L(i,j) (prefix when slot_out >= 0), 1 inverse
+ * tile W(j,i), 2 / 3 / 4 the chain tasks POTRF(j), TRSM(j) -> L(j+1,j), SYRK(j) -> A(j+1,j+1) of the first list.
+ * makespan_us (may be NULL): the cost-model estimate.  Returns the number of tasks (rows may be NULL to query
+ * it) or HSP_EINVAL.                                                                                */
+long long hsp_dbg_chol_schedule(int nt, int sb, int K, int* rows, long long capacity, double* makespan_us);
 
 #ifdef __cplusplus
 }

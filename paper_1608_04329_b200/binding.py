@@ -83,6 +83,8 @@ def lib():
     L.hsp_output_ready.argtypes = [vp, C.POINTER(ll)]
     L.hsp_output_wait.argtypes = [vp, C.POINTER(ll)]
     L.hsp_dbg_chol_trace.restype = ll
+    L.hsp_dbg_chol_schedule.argtypes = [C.c_int, C.c_int, C.c_int, vp, ll, dp]
+    L.hsp_dbg_chol_schedule.restype = ll
     _lib = L
     return L
 
@@ -286,6 +288,20 @@ class HorseshoeProbit:
         if n2 < 0:
             _check(int(n2))
         return rows
+
+
+def chol_schedule(nt, sb, K):
+    """Host-only: the static tile schedule of rows c, d1 for nt tile rows, inverse super-blocks of sb tiles, K CTAs:
+    (int32 [n_tasks, 8] = {cta, type, i, j, kbeg, kend, slot_in, slot_out}, cost-model makespan in us)."""
+    ms = C.c_double()
+    n = lib().hsp_dbg_chol_schedule(nt, sb, K, None, 0, C.byref(ms))
+    if n < 0:
+        _check(int(n))
+    rows = np.zeros((n, 8), dtype=np.int32)
+    n2 = lib().hsp_dbg_chol_schedule(nt, sb, K, _np(rows), n, C.byref(ms))
+    if n2 < 0:
+        _check(int(n2))
+    return rows, ms.value
 
 
 # ---- device unit-test hooks (torch CUDA tensors in, torch CUDA tensors out) -------------------------

@@ -23,10 +23,13 @@
 // accumulated in ascending k by a fixed sequence of tasks: the result does not depend on the number of CTAs.
 //
 // Tile products run on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> SASS DMMA; tcgen05 has no f64 kind):
-// 8 warps x (32 rows x 16 columns) of the 64x64 accumulator, operands staged by a 3-stage cp.async pipeline
-// in 32-column chunks with a padded row stride that makes the fragment loads conflict-free.
+// 8 warps x (32 rows x 16 columns) of the 64x64 accumulator.  Operands are staged in 32-column chunks by a PRODUCER WARP
+// (cp.async.bulk, one 256-byte copy per tile row into a padded row stride that makes the fragment loads
+// conflict-free; 4-stage ring, full / empty mbarriers).  The producer also does all the flag polling for the k-loops and
+// runs ahead of the compute warps across tasks, so the next task's operands arrive during this task's epilogue.
 //
 // Storage: row-major, leading dimension P; L lower, W lower, Wt upper.
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <cstdlib>
@@ -38,13 +41,19 @@ namespace hsp {
 
 constexpr int CT = 64;                 // tile edge
 constexpr int KC = 32;                 // k-columns per pipeline chunk
-constexpr int CLD = KC + 4;            // chunk row stride in doubles (288 B): conflict-free 64-bit fragment loads
+constexpr int KB = 16;                 // k-columns per TMA box: 128 bytes, the span of the 128-byte swizzle
+constexpr int kBoxBytes = CT * KB * 8; // one box: 64 tile rows x 16 k-columns of doubles = 8 KB (1024-byte aligned in shared memory)
 constexpr int TLD = CT + 4;            // full-tile row stride in shared memory (544 B)
-constexpr int NST = 3;                 // cp.async pipeline stages
-constexpr int kCholThreads = 256;
-constexpr int kStageDoubles = 2 * CT * CLD;                       // A chunk + B chunk
-constexpr int kPoolDoubles = NST * kStageDoubles;
-constexpr size_t kCholSmem = (size_t)(kPoolDoubles + 2 * CT * TLD + CT) * sizeof(double);   // pool + S + X + rdiag
+constexpr int NST = 4;                 // stages of the operand ring (bulk copies, full / empty mbarriers)
+constexpr int kCholThreads = 256;      // COMPUTE threads: 8 warps (16 warps with 16 x 16 warp tiles measured no faster)
+constexpr int kCholWarps = kCholThreads / 32;
+constexpr int kCholBlock = kCholThreads + 32;   // + the producer warp
+constexpr int kMB = CT * CT / (kCholWarps * 16) / 8;   // 8-row blocks of a warp's accumulator: (8 kMB rows) x 16 columns per warp
+constexpr int kStageBytes = 2 * (KC / KB) * kBoxBytes;            // A chunk + B chunk: 32 KB
+constexpr int kPoolDoubles = NST * kStageBytes / 8;
+constexpr uint32_t kStageTxBytes = (uint32_t)kStageBytes;   // bytes a full stage receives (A chunk + B chunk)
+// 1 KB of slack (the ring is aligned to 1024 bytes by hand) + ring + S + X + rdiag + mbarriers
+constexpr size_t kCholSmem = 1024 + (size_t)(kPoolDoubles + 2 * CT * TLD + CT) * sizeof(double) + 2 * NST * sizeof(unsigned long long);
 
 int chol_tiles(int p) { return (p + CT - 1) / CT; }
 int chol_ld(int p) { return chol_tiles(p) * CT; }
@@ -70,14 +79,49 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
   return t;
 }
+// The 8 compute warps synchronise among themselves (named barrier 1); the producer warp never joins.
+__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kCholThreads) : "memory"); }
 // Flag protocol (the pattern of a CTA-wide semaphore): the producer CTA finishes its global stores, __syncthreads(), and
-// ONE thread publishes with st.release.gpu; the consumer polls with ld.acquire.gpu from ONE thread (or the lanes of ONE
-// warp, for many flags at once) and then __syncthreads().  An acquire load costs an L1 invalidation (SASS CCTL.IVALL);
+// ONE thread publishes with st.release.gpu; the consumer polls with ld.acquire.gpu from ONE thread (or the lanes of the
+// producer warp, for many flags at once) and then synchronises the CTA (barrier / mbarrier).  An acquire load costs an L1 invalidation (SASS CCTL.IVALL);
 // polled by every warp before every k-tile it was 20 % of the kernel's stall samples at p = 4000.
 __device__ __forceinline__ void wait_flag_cta(const int* f, int tid) {
   if (tid == 0)
     while (ld_acquire(f) == 0) __nanosleep(20);
-  __syncthreads();
+  cta_sync();
+}
+__device__ __forceinline__ void cmbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void cmbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void cmbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cmbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred P1;\n\t"
+      "CWAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+      "@P1 bra CDONE;\n\t"
+      "bra CWAIT_LOOP;\n\t"
+      "CDONE:\n\t"
+      "}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+// One box of a row-major P x P matrix of doubles (tensor map: 16 columns x 64 rows, 128-byte swizzle) -> shared memory.
+__device__ __forceinline__ void tma_box(uint32_t dst_smem, const CUtensorMap* tm, int col, int row, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst_smem),
+               "l"(reinterpret_cast<uint64_t>(tm)), "r"(col), "r"(row), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ double lds_f64(uint32_t a) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+  return v;
 }
 __device__ __forceinline__ void cp_async16_s(uint32_t dst_smem, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
@@ -95,25 +139,57 @@ struct Frag {
   int row0, col0, g, t;
   __device__ __forceinline__ explicit Frag(int tid) {
     const int w = tid >> 5, lane = tid & 31;
-    row0 = (w & 1) * 32; col0 = (w >> 1) * 16; g = lane >> 2; t = lane & 3;
+    constexpr int WR = CT / (8 * kMB);   // warps along the rows
+    row0 = (w % WR) * 8 * kMB; col0 = (w / WR) * 16; g = lane >> 2; t = lane & 3;
   }
 };
 
 // acc[m][n] += sgn * sum_k A[m][k] B[n][k],  k in [0, K): A and B are row-major [row][k] in shared memory.
 template <int LDA, int LDB, int K, bool NEG>
 __device__ __forceinline__ void tile_mma(const double* __restrict__ A, const double* __restrict__ B, const Frag& f,
-                                         double (&acc)[4][2][2]) {
+                                         double (&acc)[kMB][2][2]) {
   const double* ap = A + (f.row0 + f.g) * LDA + f.t;
   const double* bp = B + (f.col0 + f.g) * LDB + f.t;
 #pragma unroll
   for (int kk = 0; kk < K; kk += 4) {
-    double a[4], b[2];
+    double a[kMB], b[2];
 #pragma unroll
-    for (int mb = 0; mb < 4; ++mb) { a[mb] = ap[mb * 8 * LDA + kk]; if (NEG) a[mb] = -a[mb]; }
+    for (int mb = 0; mb < kMB; ++mb) { a[mb] = ap[mb * 8 * LDA + kk]; if (NEG) a[mb] = -a[mb]; }
 #pragma unroll
     for (int nb = 0; nb < 2; ++nb) b[nb] = bp[nb * 8 * LDB + kk];
 #pragma unroll
-    for (int mb = 0; mb < 4; ++mb)
+    for (int mb = 0; mb < kMB; ++mb)
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb) dmma(acc[mb][nb], a[mb], b[nb]);
+  }
+}
+
+// The k-loop version: operands are TMA boxes in shared memory (32-bit shared-window addresses A, B: KC / 16 boxes each, a
+// box = 64 rows x 128 bytes with the 128-byte swizzle: the 16-byte unit u of row r sits at unit u ^ (r & 7)).  A lane
+// reads element (row0 + 8 mb + g, kk + t): its row has r & 7 = g whatever mb, so the four swizzled offsets of a box
+// (kk mod 16 = 0, 4, 8, 12) are per-lane constants `sw`.  The 32 lanes of an LDS.64 touch every 16-byte bank group exactly twice
+// (rows g and g ^ 1): two wavefronts for 256 bytes, i.e. conflict-free.
+struct SwzFrag {
+  uint32_t a0, b0, sw[4];
+  __device__ __forceinline__ explicit SwzFrag(const Frag& f) {
+    a0 = (uint32_t)((f.row0 + f.g) * 128);
+    b0 = (uint32_t)((f.col0 + f.g) * 128);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) sw[q] = (uint32_t)((((2 * q + (f.t >> 1)) ^ f.g) * 16) + (f.t & 1) * 8);
+  }
+};
+template <bool NEG>
+__device__ __forceinline__ void tile_mma_s(uint32_t A, uint32_t B, const SwzFrag& z, double (&acc)[kMB][2][2]) {
+#pragma unroll
+  for (int kk = 0; kk < KC; kk += 4) {
+    const uint32_t o = (uint32_t)((kk / KB) * kBoxBytes) + z.sw[(kk % KB) / 4];
+    double a[kMB], b[2];
+#pragma unroll
+    for (int mb = 0; mb < kMB; ++mb) { a[mb] = lds_f64(A + z.a0 + (uint32_t)(mb * 8 * 128) + o); if (NEG) a[mb] = -a[mb]; }
+#pragma unroll
+    for (int nb = 0; nb < 2; ++nb) b[nb] = lds_f64(B + z.b0 + (uint32_t)(nb * 8 * 128) + o);
+#pragma unroll
+    for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
       for (int nb = 0; nb < 2; ++nb) dmma(acc[mb][nb], a[mb], b[nb]);
   }
@@ -129,7 +205,7 @@ __device__ __forceinline__ double fast_rcp(double d) {
   return fma(r, t, r);
 }
 
-// In-place Cholesky of the 64x64 tile S (stride TLD, lower triangle used), all 256 threads; on return the
+// In-place Cholesky of the 64x64 tile S (stride TLD, lower triangle used), every thread of the CTA; on return the
 // lower triangle of S holds L (diagonal included) and rdiag[r] = 1 / L_rr.  Blocked by 16 columns: the
 // 16-column panel below and including the diagonal block is factored in registers, 32 rows per warp (lanes
 // 0-15 hold the diagonal block -- redundantly in every warp --, lanes 16-31 sixteen panel rows).  A pivot
@@ -188,7 +264,7 @@ __device__ __forceinline__ bool tile_potrf(double* __restrict__ S, double* __res
         }
       }
     }
-    __syncthreads();
+    cta_sync();
     if (npanel > 0) {
       // trailing update: S[r][c] -= sum_{m<16} S[r][o+m] S[c][o+m] for o+16 <= c <= r < 64, 8x8 blocks
       const int o2 = o + 16, nb8 = npanel / 8, g = lane >> 2, t = lane & 3;
@@ -219,7 +295,7 @@ __device__ __forceinline__ bool tile_potrf(double* __restrict__ S, double* __res
         for (int u = 0; u < 3; ++u)
           if (on[u]) *reinterpret_cast<double2*>(cp[u]) = make_double2(c[u][0], c[u][1]);
       }
-      __syncthreads();
+      cta_sync();
     }
   }
   return ok;
@@ -251,7 +327,7 @@ __device__ __forceinline__ void tile_trinv(const double* __restrict__ S, const d
                                            double* __restrict__ X, int tid) {
   const int warp = tid >> 5, lane = tid & 31;
   for (int e = tid; e < CT * TLD / 2; e += kCholThreads) reinterpret_cast<double2*>(X)[e] = make_double2(0.0, 0.0);
-  __syncthreads();
+  cta_sync();
   if (tid < CT) {
     const int b0 = (tid >> 4) * 16, c = tid & 15;
     double x[16];
@@ -267,56 +343,125 @@ __device__ __forceinline__ void tile_trinv(const double* __restrict__ S, const d
 #pragma unroll
     for (int r = 0; r < 16; ++r) X[(b0 + r) * TLD + b0 + c] = x[r];
   }
-  __syncthreads();
+  cta_sync();
   {
-    // h = 16: the two 32x32 diagonal blocks, four warps each
-    const int off = (warp >> 2) * 32, w = warp & 3;
-    sub_mma<16>(S + (off + 16) * TLD + off, X + off * TLD + off, X + off * TLD + off + 16, false, w, 4, lane);      // T = B A^-1
-    __syncthreads();
-    sub_mma<16>(X + (off + 16) * TLD + off + 16, X + off * TLD + off + 16, X + (off + 16) * TLD + off, true, w, 4, lane);   // -C^-1 T
-    __syncthreads();
+    // h = 16: the two 32x32 diagonal blocks, half of the warps each
+    const int off = (warp / (kCholWarps / 2)) * 32, w = warp % (kCholWarps / 2);
+    sub_mma<16>(S + (off + 16) * TLD + off, X + off * TLD + off, X + off * TLD + off + 16, false, w, kCholWarps / 2, lane);      // T = B A^-1
+    cta_sync();
+    sub_mma<16>(X + (off + 16) * TLD + off + 16, X + off * TLD + off + 16, X + (off + 16) * TLD + off, true, w, kCholWarps / 2, lane);   // -C^-1 T
+    cta_sync();
     for (int e = tid; e < 2 * 16 * 16; e += kCholThreads) {
       const int blk = e >> 8, r = (e >> 4) & 15, c = e & 15;
       X[(blk * 32 + r) * TLD + blk * 32 + 16 + c] = 0.0;
     }
-    __syncthreads();
+    cta_sync();
   }
   {
     // h = 32
-    sub_mma<32>(S + 32 * TLD, X, X + 32, false, warp, 8, lane);
-    __syncthreads();
-    sub_mma<32>(X + 32 * TLD + 32, X + 32, X + 32 * TLD, true, warp, 8, lane);
-    __syncthreads();
+    sub_mma<32>(S + 32 * TLD, X, X + 32, false, warp, kCholWarps, lane);
+    cta_sync();
+    sub_mma<32>(X + 32 * TLD + 32, X + 32, X + 32 * TLD, true, warp, kCholWarps, lane);
+    cta_sync();
     for (int e = tid; e < 32 * 32; e += kCholThreads) X[(e >> 5) * TLD + 32 + (e & 31)] = 0.0;
-    __syncthreads();
+    cta_sync();
   }
 }
 
-__global__ void __launch_bounds__(kCholThreads, 1)
+__global__ void __launch_bounds__(kCholBlock, 1)
 chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_inv2, Ctl* __restrict__ ctl,
                  double* __restrict__ L, double* __restrict__ W, double* __restrict__ Wt, double* __restrict__ ws,
                  int* __restrict__ flags, const CholTask* __restrict__ tasks, const int* __restrict__ list_off, int p,
-                 int nt, unsigned long long* __restrict__ trace, double* __restrict__ Lt) {
-  extern __shared__ __align__(16) double pool[];
+                 int nt, unsigned long long* __restrict__ trace, double* __restrict__ Lt,
+                 const __grid_constant__ CUtensorMap tmL, const __grid_constant__ CUtensorMap tmWt) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  // the operand ring must be 1024-byte aligned (128-byte swizzle atom = 8 rows x 128 bytes)
+  double* pool = reinterpret_cast<double*>(smem_raw + ((1024u - ((uint32_t)__cvta_generic_to_shared(smem_raw) & 1023u)) & 1023u));
   double* S = pool + kPoolDoubles;                   // 64 x TLD
   double* X = S + CT * TLD;                          // 64 x TLD
   double* rdiag = X + CT * TLD;                      // 64
-  __shared__ int s_ready[2];                         // result of the last two flag scans (double-buffered)
   const int P = nt * CT;
   const int tid = threadIdx.x;
-  const Frag f(tid);
   const uint32_t pool_s = (uint32_t)__cvta_generic_to_shared(pool);
   const uint32_t x_s = pool_s + (uint32_t)((kPoolDoubles + CT * TLD) * sizeof(double));
-  int scan_par = 0;
+  const uint32_t bar_s = pool_s + (uint32_t)((kPoolDoubles + 2 * CT * TLD + CT) * sizeof(double));   // full[NST], empty[NST]
   int* fL = flags;
   int* fB = flags + (size_t)nt * nt;
   int* fP = fB + (size_t)nt * nt;
+  if (tid == 0) {
+    for (int q = 0; q < NST; ++q) {
+      cmbar_init(bar_s + 8u * q, 1);                       // full: the producer's arrive.expect_tx (+ the bytes)
+      cmbar_init(bar_s + 8u * (NST + q), kCholWarps);      // empty: one arrival per compute warp
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();                                         // the only CTA-wide barrier: the producer warp leaves here
+  const int t_beg = list_off[blockIdx.x], t_end = list_off[blockIdx.x + 1];
+
+  if (tid >= kCholThreads) {
+    // ---- producer warp: for every k-loop of this CTA's list, in order: wait for the operands' flags (the lanes look at
+    // up to 32 k-tiles at once), wait for a free stage, and stream the two 64 x 32 operand chunks into it: four 2-D TMA
+    // boxes (cp.async.bulk.tensor, 128-byte swizzle), issued by one lane.
+    const int lane = tid & 31;
+    uint32_t st = 0, ph = 0;
+    for (int ti = t_beg; ti < t_end; ++ti) {
+      const CholTask tk = tasks[ti];
+      if (tk.type >= 2 || tk.kend <= tk.kbeg) continue;
+      const bool isL = tk.type == 0;
+      const int ra = isL ? tk.i : tk.j, rb = isL ? tk.j : tk.i;
+      int k_known = tk.kbeg;                               // k-tiles below this are known to be ready
+      for (int k = tk.kbeg; k < tk.kend; ++k) {
+        if (k >= k_known) {
+          // operand flags of k-tile kq: L(ra,kq) and L(rb,kq) (L tasks), L(ra,kq) and Wt(rb,kq) (inverse tiles)
+          const int kq = k + lane;
+          int n;
+          for (;;) {
+            bool ok = false;
+            if (kq < tk.kend) {
+              ok = ld_acquire(&fL[(size_t)ra * nt + kq]) != 0;
+              if (isL) { if (rb != ra) ok = (ld_acquire(&fL[(size_t)rb * nt + kq]) != 0) && ok; }
+              else ok = (ld_acquire(kq == rb ? &fL[(size_t)rb * nt + rb] : &fB[(size_t)rb * nt + kq]) != 0) && ok;
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, ok);
+            n = __ffs(~m) - 1;
+            if (n < 0) n = 32;
+            if (n > 0) break;
+            __nanosleep(20);
+          }
+          k_known = k + n;
+          // the tiles were written through the generic proxy by other CTAs; the bulk copies read through the async proxy
+          asm volatile("fence.proxy.async.global;" ::: "memory");
+        }
+#pragma unroll 1
+        for (int kc = 0; kc < CT / KC; ++kc) {
+          const uint32_t full = bar_s + 8u * st, empty = bar_s + 8u * (NST + st);
+          cmbar_wait(empty, ph ^ 1u);
+          if (lane == 0) cmbar_expect_tx(full, kStageTxBytes);
+          if (lane == 0) {
+            const uint32_t sa = pool_s + st * (uint32_t)kStageBytes;
+            const uint32_t sb = sa + (uint32_t)((KC / KB) * kBoxBytes);
+#pragma unroll
+            for (int q = 0; q < KC / KB; ++q) {
+              tma_box(sa + (uint32_t)(q * kBoxBytes), &tmL, k * CT + kc * KC + q * KB, ra * CT, full);
+              tma_box(sb + (uint32_t)(q * kBoxBytes), isL ? &tmL : &tmWt, k * CT + kc * KC + q * KB, rb * CT, full);
+            }
+          }
+          if (++st == NST) { st = 0; ph ^= 1u; }
+        }
+      }
+    }
+    return;
+  }
+
+  const Frag f(tid);
+  const SwzFrag zf(f);
+  uint32_t c_st = 0, c_ph = 0;                             // the compute warps' position in the ring
   const double tau_inv2 = ctl->tau_inv2;
 
   // c: the Q tile (ti, tj) in the accumulator layout, padded with the identity
-  auto load_q_tile = [&](int ti_, int tj_, double (&a)[4][2][2]) {
+  auto load_q_tile = [&](int ti_, int tj_, double (&a)[kMB][2][2]) {
 #pragma unroll
-    for (int mb = 0; mb < 4; ++mb)
+    for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
       for (int nb = 0; nb < 2; ++nb)
 #pragma unroll
@@ -330,18 +475,18 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
           a[mb][nb][e] = v;
         }
   };
-  auto load_slot = [&](int slot, double (&a)[4][2][2]) {
+  auto load_slot = [&](int slot, double (&a)[kMB][2][2]) {
     wait_flag_cta(&fP[slot], tid);
     const double2* src = reinterpret_cast<const double2*>(ws + (size_t)slot * CT * CT);
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
+    for (int q = 0; q < 2 * kMB; ++q) {
       const double2 v = __ldcg(src + q * kCholThreads + tid);
       a[q >> 1][q & 1][0] = v.x; a[q >> 1][q & 1][1] = v.y;
     }
   };
-  auto acc_to_smem = [&](const double (&a)[4][2][2], double* T) {
+  auto acc_to_smem = [&](const double (&a)[kMB][2][2], double* T) {
 #pragma unroll
-    for (int mb = 0; mb < 4; ++mb)
+    for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
       for (int nb = 0; nb < 2; ++nb)
         *reinterpret_cast<double2*>(T + (f.row0 + mb * 8 + f.g) * TLD + f.col0 + nb * 8 + 2 * f.t) = make_double2(a[mb][nb][0], a[mb][nb][1]);
@@ -363,53 +508,52 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       if (Lt != nullptr)   // L^T, used by the block back-substitution when only a block-diagonal inverse is built
         *reinterpret_cast<double2*>(Lt + g) = make_double2(c >= r ? S[c * TLD + r] : 0.0, c + 1 >= r ? S[(c + 1) * TLD + r] : 0.0);
     }
-    __syncthreads();
+    cta_sync();
     if (tid == 0) st_release(&fL[(size_t)j_ * nt + j_], 1);
   };
 
-  const int t_end = list_off[blockIdx.x + 1];
-  for (int ti = list_off[blockIdx.x]; ti < t_end; ++ti) {
+  for (int ti = t_beg; ti < t_end; ++ti) {
     const CholTask tk = tasks[ti];
     if (trace != nullptr && tid == 0) trace[4 * (size_t)ti] = globaltimer_ns();
     if (tk.type >= 2) {
       // ---- chain tasks (dedicated CTA; S, X persist in shared memory from one chain task to the next)
       const int j = tk.j;
-      double acc[4][2][2];
+      double acc[kMB][2][2];
       if (tk.type == 2) {
         // POTRF(j): S holds A_jj (left there by SYRK(j-1); column 0: the Q tile)
         if (j == 0) { load_q_tile(0, 0, acc); acc_to_smem(acc, S); }
-        __syncthreads();
+        cta_sync();
         diag_finish(j);
       } else if (tk.type == 3) {
         // TRSM(j): L(j+1,j) = A W_jj^T, A = parked accumulator of (j+1,j) with every k < j applied (column 0: Q tile);
         // W_jj is still in X.  The product goes to global memory and stays in S as the operand of SYRK(j).
         if (tk.slot_in >= 0) load_slot(tk.slot_in, acc); else load_q_tile(j + 1, j, acc);
-        __syncthreads();                              // everyone is done with S (L_jj was written out by POTRF(j))
+        cta_sync();                              // everyone is done with S (L_jj was written out by POTRF(j))
         acc_to_smem(acc, S);
-        __syncthreads();
-        double out[4][2][2];
+        cta_sync();
+        double out[kMB][2][2];
 #pragma unroll
-        for (int mb = 0; mb < 4; ++mb)
+        for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb) out[mb][nb][0] = out[mb][nb][1] = 0.0;
         tile_mma<TLD, TLD, CT, false>(S, X, f, out);
 #pragma unroll
-        for (int mb = 0; mb < 4; ++mb)
+        for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb) {
             const int r = (j + 1) * CT + f.row0 + mb * 8 + f.g, c = j * CT + f.col0 + nb * 8 + 2 * f.t;
             *reinterpret_cast<double2*>(L + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
             if (Lt != nullptr) { Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1]; }
           }
-        __syncthreads();                              // the product has been read from S by every warp
+        cta_sync();                              // the product has been read from S by every warp
         acc_to_smem(out, S);
-        __syncthreads();
+        cta_sync();
         if (tid == 0) st_release(&fL[(size_t)(j + 1) * nt + j], 1);
       } else {
         // SYRK(j): A(j+1,j+1) = parked accumulator (every k < j applied; column 1: Q tile) - L(j+1,j) L(j+1,j)^T -> S
         if (tk.slot_in >= 0) load_slot(tk.slot_in, acc); else load_q_tile(j + 1, j + 1, acc);
         tile_mma<TLD, TLD, CT, true>(S, S, f, acc);
-        __syncthreads();
+        cta_sync();
         acc_to_smem(acc, S);
       }
       if (trace != nullptr && tid == 0) {
@@ -420,120 +564,71 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
     }
     const bool isL = tk.type == 0;
     const int i = tk.i, j = tk.j;
-    // operands of the k loop: acc -= MA(ra,k) MB(rb,k)^T
-    const double* MA = L;
-    const double* MB = isL ? L : Wt;
-    const int ra = isL ? i : j, rb = isL ? j : i;
+    // the k loop: acc -= MA(ra,k) MB(rb,k)^T, operands streamed by the producer warp
     const int kbeg = tk.kbeg, kend = tk.kend;
 
-    double acc[4][2][2];
+    double acc[kMB][2][2];
     if (tk.slot_in >= 0) load_slot(tk.slot_in, acc);
     else if (isL) load_q_tile(i, j, acc);
     else {
 #pragma unroll
-      for (int mb = 0; mb < 4; ++mb)
+      for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
         for (int nb = 0; nb < 2; ++nb) acc[mb][nb][0] = acc[mb][nb][1] = 0.0;
     }
 
     const int nchunks = (kend - kbeg) * (CT / KC);
-    // operand flags of k-tile k: L(ra,k) and L(rb,k) (L tasks), L(ra,k) and Wt(rb,k) (inverse tiles)
-    auto k_ready = [&](int k) -> bool {
-      bool ok = ld_acquire(&fL[(size_t)ra * nt + k]) != 0;
-      if (isL) { if (rb != ra) ok = (ld_acquire(&fL[(size_t)rb * nt + k]) != 0) && ok; }
-      else ok = (ld_acquire(k == rb ? &fL[(size_t)rb * nt + rb] : &fB[(size_t)rb * nt + k]) != 0) && ok;
-      return ok;
-    };
-    // warp 0 looks at the flags of up to 32 k-tiles from k0 on (a lane each), spins until k0 itself is ready and
-    // publishes the first k that is NOT known to be ready; every thread returns it
-    auto scan = [&](int k0) -> int {
-      scan_par ^= 1;
-      if (tid < 32) {
-        const int k = k0 + tid;
-        int n;
-        for (;;) {
-          const bool ok = k < kend ? k_ready(k) : false;
-          const unsigned m = __ballot_sync(0xffffffffu, ok);
-          n = __ffs(~m) - 1;
-          if (n < 0) n = 32;
-          if (n > 0) break;
-          __nanosleep(20);
-        }
-        if (tid == 0) s_ready[scan_par] = k0 + n;
-      }
-      __syncthreads();
-      return s_ready[scan_par];
-    };
-    int k_known = kbeg;                              // k-tiles below this are known to be ready
-    const int ld_row = tid >> 4, ld_pc = (tid & 15) * 2;
-    auto issue = [&](int c) {
-      const int k = kbeg + c / (CT / KC), kc = c % (CT / KC);
-      if (kc == 0 && k >= k_known) k_known = scan(k);   // first chunk of a k tile: its producers must be done
-      const uint32_t sa = pool_s + (uint32_t)((c % NST) * kStageDoubles * sizeof(double)) + (uint32_t)((ld_row * CLD + ld_pc) * sizeof(double));
-      const uint32_t sb = sa + (uint32_t)(CT * CLD * sizeof(double));
-      const double* ga = MA + (size_t)ra * CT * P + (size_t)k * CT + kc * KC + (size_t)ld_row * P + ld_pc;
-      const double* gb = MB + (size_t)rb * CT * P + (size_t)k * CT + kc * KC + (size_t)ld_row * P + ld_pc;
-#pragma unroll
-      for (int it = 0; it < CT / 16; ++it) {
-        cp_async16_s(sa + (uint32_t)(it * 16 * CLD * sizeof(double)), ga + (size_t)it * 16 * P);
-        cp_async16_s(sb + (uint32_t)(it * 16 * CLD * sizeof(double)), gb + (size_t)it * 16 * P);
-      }
-    };
-    __syncthreads();                                 // the pool, S and X are free (previous task is over)
-    for (int c = 0; c < NST - 1; ++c) {
-      if (c < nchunks) issue(c);
-      cp_async_commit();
-    }
+    cta_sync();                                      // S and X are free (previous task is over)
+#pragma unroll 1
     for (int c = 0; c < nchunks; ++c) {
-      cp_async_wait<NST - 2>();
-      __syncthreads();
-      if (c + NST - 1 < nchunks) issue(c + NST - 1);
-      cp_async_commit();
-      const double* sa = pool + (size_t)(c % NST) * kStageDoubles;
-      tile_mma<CLD, CLD, KC, true>(sa, sa + CT * CLD, f, acc);
+      cmbar_wait(bar_s + 8u * c_st, c_ph);
+      const uint32_t sa = pool_s + c_st * (uint32_t)kStageBytes;
+      tile_mma_s<true>(sa, sa + (uint32_t)((KC / KB) * kBoxBytes), zf, acc);
+      __syncwarp();
+      if ((tid & 31) == 0) cmbar_arrive(bar_s + 8u * (NST + c_st));
+      if (++c_st == NST) { c_st = 0; c_ph ^= 1u; }
     }
-    cp_async_wait<0>();
     if (trace != nullptr && tid == 0) trace[4 * (size_t)ti + 1] = globaltimer_ns();
 
     if (tk.slot_out >= 0) {
       // ---- prefix task: park the partial accumulator
       double2* dst = reinterpret_cast<double2*>(ws + (size_t)tk.slot_out * CT * CT);
 #pragma unroll
-      for (int q = 0; q < 8; ++q) __stcg(dst + q * kCholThreads + tid, make_double2(acc[q >> 1][q & 1][0], acc[q >> 1][q & 1][1]));
-      __syncthreads();
+      for (int q = 0; q < 2 * kMB; ++q) __stcg(dst + q * kCholThreads + tid, make_double2(acc[q >> 1][q & 1][0], acc[q >> 1][q & 1][1]));
+      cta_sync();
       if (tid == 0) st_release(&fP[tk.slot_out], 1);
     } else if (isL && i == j) {
       // ---- diagonal: L_jj = chol(acc), W_jj = L_jj^-1
       acc_to_smem(acc, S);
-      __syncthreads();
+      cta_sync();
       diag_finish(j);
     } else {
       // ---- off-diagonal: multiply by W_jj (from global; written by the diagonal task of column j)
       wait_flag_cta(&fL[(size_t)j * nt + j], tid);
       const double* wjj = W + (size_t)j * CT * P + (size_t)j * CT;
 #pragma unroll
-      for (int it = 0; it < CT / 8; ++it) {
-        const int row = (tid >> 5) + it * 8, pc = (tid & 31) * 2;
+      for (int it = 0; it < CT / kCholWarps; ++it) {
+        const int row = (tid >> 5) + it * kCholWarps, pc = (tid & 31) * 2;
         cp_async16_s(x_s + (uint32_t)((row * TLD + pc) * sizeof(double)), wjj + (size_t)row * P + pc);
       }
       cp_async_commit();
-      double out[4][2][2];
+      double out[kMB][2][2];
 #pragma unroll
-      for (int mb = 0; mb < 4; ++mb)
+      for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
         for (int nb = 0; nb < 2; ++nb) out[mb][nb][0] = out[mb][nb][1] = 0.0;
       if (isL) {
 #pragma unroll
-        for (int mb = 0; mb < 4; ++mb)
+        for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb)
             *reinterpret_cast<double2*>(S + (f.row0 + mb * 8 + f.g) * TLD + f.col0 + nb * 8 + 2 * f.t) =
                 make_double2(acc[mb][nb][0], acc[mb][nb][1]);
         cp_async_wait<0>();
-        __syncthreads();
+        cta_sync();
         tile_mma<TLD, TLD, CT, false>(S, X, f, out);               // L_ij = A W_jj^T
 #pragma unroll
-        for (int mb = 0; mb < 4; ++mb)
+        for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb)
           {
@@ -541,21 +636,21 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
             *reinterpret_cast<double2*>(L + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
             if (Lt != nullptr) { Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1]; }
           }
-        __syncthreads();
+        cta_sync();
         if (tid == 0) st_release(&fL[(size_t)i * nt + j], 1);
       } else {
 #pragma unroll
-        for (int mb = 0; mb < 4; ++mb)
+        for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb)
 #pragma unroll
             for (int e = 0; e < 2; ++e)
               S[(f.col0 + nb * 8 + 2 * f.t + e) * TLD + f.row0 + mb * 8 + f.g] = acc[mb][nb][e];   // transposed
         cp_async_wait<0>();
-        __syncthreads();
+        cta_sync();
         tile_mma<TLD, TLD, CT, false>(X, S, f, out);               // W_ji = W_jj A
 #pragma unroll
-        for (int mb = 0; mb < 4; ++mb)
+        for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb) {
             const int r = j * CT + f.row0 + mb * 8 + f.g, c = i * CT + f.col0 + nb * 8 + 2 * f.t;
@@ -563,7 +658,7 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
             Wt[(size_t)c * P + r] = out[mb][nb][0];
             Wt[(size_t)(c + 1) * P + r] = out[mb][nb][1];
           }
-        __syncthreads();
+        cta_sync();
         if (tid == 0) st_release(&fB[(size_t)i * nt + j], 1);
       }
     }
@@ -747,6 +842,8 @@ beta_keep_kernel(const double* __restrict__ beta, int p, Ctl* __restrict__ ctl) 
 // Build the static schedule and decide how many SMs the Cholesky branch gets.  When the cost model says the
 // branch hides behind the fused pass on K SMs of its own (the pass keeps num_sms - K), the smallest such K
 // is taken; otherwise the branch uses every SM and runs before/after the pass.
+static cudaError_t make_tile_map(CUtensorMap* tm, const double* base, int P);
+
 cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_estimate, const Options& opt) {
   pl->p = p; pl->nt = chol_tiles(p); pl->P = chol_ld(p);
   const int nt = pl->nt;
@@ -824,6 +921,10 @@ cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_e
   }
   pl->h_tasks = best.tasks;
   if (e == cudaSuccess) e = cudaFuncSetAttribute(chol_task_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCholSmem);
+  if (e == cudaSuccess) {   // look the driver's tensor-map encoder up now, outside any stream capture
+    CUtensorMap probe;
+    e = make_tile_map(&probe, pl->d_ws, 64);
+  }
   return e;
 }
 
@@ -836,16 +937,45 @@ void chol_plan_destroy(CholPlan* pl) {
   *pl = CholPlan{};
 }
 
+// Tensor map of a row-major P x P matrix of doubles for boxes of 16 columns x 64 rows with the 128-byte swizzle.  The
+// driver entry point is looked up through the runtime (libhsp.so links only cudart).
+static cudaError_t make_tile_map(CUtensorMap* tm, const double* base, int P) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    const cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return e;
+    if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+    encode = reinterpret_cast<EncodeFn>(fn);
+  }
+  const cuuint64_t gdim[2] = {(cuuint64_t)P, (cuuint64_t)P};
+  const cuuint64_t gstride[1] = {(cuuint64_t)P * sizeof(double)};
+  const cuuint32_t box[2] = {(cuuint32_t)KB, (cuuint32_t)CT};
+  const cuuint32_t estride[2] = {1, 1};
+  const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), gdim, gstride, box, estride,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 cudaError_t cholesky_launch(const CholPlan& pl, const double* G, const double* lam_inv2, Ctl* ctl, double* L, double* W,
                             double* Wt, double* Lt, cudaStream_t st, long long* launches) {
   cudaError_t e = cudaMemsetAsync(pl.d_flags, 0, pl.n_flags * sizeof(int), st);
   if (e != cudaSuccess) return e;
   int p = pl.p, nt = pl.nt;
+  CUtensorMap tmL, tmWt;
+  e = make_tile_map(&tmL, L, pl.P);
+  if (e == cudaSuccess) e = make_tile_map(&tmWt, Wt, pl.P);
+  if (e != cudaSuccess) return e;
   double* ws = pl.d_ws; int* flags = pl.d_flags; const CholTask* tasks = pl.d_tasks; const int* list_off = pl.d_list_off;
   unsigned long long* trace = pl.d_trace;
   void* args[] = {(void*)&G, (void*)&lam_inv2, (void*)&ctl, (void*)&L, (void*)&W, (void*)&Wt, (void*)&ws, (void*)&flags,
-                  (void*)&tasks, (void*)&list_off, (void*)&p, (void*)&nt, (void*)&trace, (void*)&Lt};
-  e = cudaLaunchCooperativeKernel((const void*)chol_task_kernel, dim3(pl.K), dim3(kCholThreads), args, kCholSmem, st);
+                  (void*)&tasks, (void*)&list_off, (void*)&p, (void*)&nt, (void*)&trace, (void*)&Lt, (void*)&tmL, (void*)&tmWt};
+  e = cudaLaunchCooperativeKernel((const void*)chol_task_kernel, dim3(pl.K), dim3(kCholBlock), args, kCholSmem, st);
   if (launches) ++*launches;
   return e;
 }

@@ -757,6 +757,22 @@ long long hsp_dbg_chol_trace(const hsp_state* s, long long* rows, long long capa
   return n;
 }
 
+long long hsp_dbg_chol_schedule(int nt, int sb, int K, int* rows, long long capacity, double* makespan_us) {
+  if (nt < 1 || sb < 1 || K < 1 || (long long)K > (long long)nt * nt) return fail(HSP_EINVAL, "hsp_dbg_chol_schedule: need nt, sb >= 1 and 1 <= K <= nt^2");
+  const CholSchedule sc = chol_build_schedule(nt, sb > nt ? nt : sb, K);
+  const long long n = (long long)sc.tasks.size();
+  if (makespan_us) *makespan_us = sc.makespan_us;
+  if (!rows) return n;
+  if (capacity < n) return fail(HSP_EINVAL, "capacity is smaller than the number of tasks");
+  for (int k = 0; k < sc.K; ++k)
+    for (int q = sc.list_off[k]; q < sc.list_off[k + 1]; ++q) {
+      const CholTask& t = sc.tasks[(size_t)q];
+      int* r = rows + 8 * (size_t)q;
+      r[0] = k; r[1] = t.type; r[2] = t.i; r[3] = t.j; r[4] = t.kbeg; r[5] = t.kend; r[6] = t.slot_in; r[7] = t.slot_out;
+    }
+  return n;
+}
+
 // ---- device unit-test hooks ----------------------------------------------------------------------
 __global__ void dbg_philox_kernel(const unsigned* ctr, const unsigned* key, unsigned* out, long long n) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
