@@ -197,7 +197,8 @@ int hsp_dbg_cheng(double alpha, unsigned long long seed, unsigned sweep0, double
  * option "chol_trace" = 1 was in force when the chain was created, the device timestamps of
  * the tasks of the last sweep.  rows: HOST, capacity x 12 long long per task, in schedule order:
  * {type, i, j, kbeg, kend, slot_in, slot_out, cta, t_start_ns, t_kloop_end_ns, t_end_ns, 0} (timestamps 0
- * without the trace).  Returns the number of tasks (rows may be NULL to query it), or a negative status.
+ * without the trace; chain task POTRF, type 2: t_kloop_end_ns = end of the tile factorisation and the last word = end of
+ * the triangular inverse).  Returns the number of tasks (rows may be NULL to query it), or a negative status.
  * Synchronises.                                                                                     */
 long long hsp_dbg_chol_trace(const hsp_state* s, long long* rows, long long capacity);
 /* Host-only (no device needed): the static schedule the library would build for nt tile rows (64 x 64 tiles), inverse

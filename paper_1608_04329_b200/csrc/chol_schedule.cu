@@ -28,7 +28,10 @@ namespace hsp {
 
 namespace {
 
-struct Cost { double mac = 3.3, hop = 2.0, potrf = 8.0, trinv = 3.0, store = 0.9, loadp = 0.5, cmac = 2.6; };   // us, from the chol_trace option at p = 1000 (cmac: a product of the chain CTA, operands in shared memory)
+// us, from the chol_trace option at p = 1000 and p = 4000 (profiles/r02_c_cholesky.md).  mac: one 64x64x64 product of a k-loop (TMA-fed,
+// DMMA peak 2.08); fin: finish of an off-diagonal tile (wait for W_jj, load it, product, store, flag); cmac: a product of the
+// chain CTA, operands in shared memory; cpub: W_jj reaches global memory (publisher warp) that long after the inverse
+struct Cost { double mac = 2.4, hop = 2.0, potrf = 7.9, trinv = 1.9, store = 0.9, loadp = 0.3, cmac = 2.6, fin = 4.7, cpub = 0.5; };
 
 struct Step { double cost; int dep[2]; bool local = false; };   // deps are task ids (-1 = none); local: dep[0] ran on the same CTA (no flag hop)
 struct Node {
@@ -66,12 +69,12 @@ Graph build_graph(int nt, int sb, const Cost& c, bool chain) {
         g.n[pd].steps.push_back(Step{c.store, {-1, -1}});
       }
       const int po = add(CholTask{2, j, j, 0, 0, -1, -1, 0});
-      g.n[po].steps.push_back(Step{c.potrf + c.trinv + c.store, {prev, -1}, true});
+      g.n[po].steps.push_back(Step{c.potrf + c.trinv + c.cpub, {prev, -1}, true});
       g.chain.push_back(po); prev = po;
       idL[(size_t)j * nt + j] = po;
       if (j + 1 < nt) {
         const int tr = add(CholTask{3, j + 1, j, 0, 0, slot_s, -1, 0});
-        g.n[tr].steps.push_back(Step{c.loadp + c.cmac + c.store, {po, ps}, true});
+        g.n[tr].steps.push_back(Step{c.loadp + c.cmac + c.store - c.cpub, {po, ps}, true});
         g.chain.push_back(tr);
         idL[(size_t)(j + 1) * nt + j] = tr;
         const int sy = add(CholTask{4, j + 1, j, 0, 0, slot_d, -1, 0});
@@ -81,7 +84,7 @@ Graph build_graph(int nt, int sb, const Cost& c, bool chain) {
       for (int i = j + 2; i < nt; ++i) {
         const int id = add(CholTask{0, i, j, 0, j, -1, -1, 0});
         for (int k = 0; k < j; ++k) g.n[id].steps.push_back(Step{c.mac, {idL[(size_t)i * nt + k], idL[(size_t)j * nt + k]}});
-        g.n[id].steps.push_back(Step{c.mac + c.store, {po, -1}});
+        g.n[id].steps.push_back(Step{c.fin, {po, -1}});
         idL[(size_t)i * nt + j] = id;
       }
     }
@@ -101,7 +104,7 @@ Graph build_graph(int nt, int sb, const Cost& c, bool chain) {
       if (split) g.n[id].steps.push_back(Step{c.loadp, {pre, -1}});
       for (int k = k0; k < j; ++k) g.n[id].steps.push_back(Step{c.mac, {idL[(size_t)i * nt + k], i != j ? idL[(size_t)j * nt + k] : -1}});
       if (i == j) g.n[id].steps.push_back(Step{c.potrf + c.trinv + c.store, {-1, -1}});
-      else g.n[id].steps.push_back(Step{c.mac + c.store, {idL[(size_t)j * nt + j], -1}});
+      else g.n[id].steps.push_back(Step{c.fin, {idL[(size_t)j * nt + j], -1}});
       idL[(size_t)i * nt + j] = id;
     }
   // inverse tiles W(j,i), i < j, inside one super-block of sb tiles
@@ -111,7 +114,7 @@ Graph build_graph(int nt, int sb, const Cost& c, bool chain) {
       const int id = add(CholTask{1, i, j, i, j, -1, -1, 0});
       for (int k = i; k < j; ++k)
         g.n[id].steps.push_back(Step{c.mac, {idL[(size_t)j * nt + k], k == i ? idL[(size_t)i * nt + i] : idB[(size_t)i * nt + k]}});
-      g.n[id].steps.push_back(Step{c.mac + c.store, {idL[(size_t)j * nt + j], -1}});
+      g.n[id].steps.push_back(Step{c.fin, {idL[(size_t)j * nt + j], -1}});
       idB[(size_t)i * nt + j] = id;
     }
   for (size_t a = 0; a < g.n.size(); ++a) {

@@ -47,13 +47,14 @@ constexpr int TLD = CT + 4;            // full-tile row stride in shared memory 
 constexpr int NST = 4;                 // stages of the operand ring (bulk copies, full / empty mbarriers)
 constexpr int kCholThreads = 256;      // COMPUTE threads: 8 warps (16 warps with 16 x 16 warp tiles measured no faster)
 constexpr int kCholWarps = kCholThreads / 32;
-constexpr int kCholBlock = kCholThreads + 32;   // + the producer warp
+constexpr int kCholBlock = kCholThreads + 64;   // + the producer warp + the publisher warp (chain CTA)
+constexpr int kChainStages = 2;        // ring stages the chain CTA uses for its parked accumulators; the rest of the ring holds its third tile buffer
 constexpr int kMB = CT * CT / (kCholWarps * 16) / 8;   // 8-row blocks of a warp's accumulator: (8 kMB rows) x 16 columns per warp
 constexpr int kStageBytes = 2 * (KC / KB) * kBoxBytes;            // A chunk + B chunk: 32 KB
 constexpr int kPoolDoubles = NST * kStageBytes / 8;
 constexpr uint32_t kStageTxBytes = (uint32_t)kStageBytes;   // bytes a full stage receives (A chunk + B chunk)
 // 1 KB of slack (the ring is aligned to 1024 bytes by hand) + ring + S + X + rdiag + mbarriers
-constexpr size_t kCholSmem = 1024 + (size_t)(kPoolDoubles + 2 * CT * TLD + CT) * sizeof(double) + 2 * NST * sizeof(unsigned long long);
+constexpr size_t kCholSmem = 1024 + (size_t)(kPoolDoubles + 2 * CT * TLD + CT) * sizeof(double) + (2 * NST + 4) * sizeof(unsigned long long);
 
 int chol_tiles(int p) { return (p + CT - 1) / CT; }
 int chol_ld(int p) { return chol_tiles(p) * CT; }
@@ -117,6 +118,16 @@ __device__ __forceinline__ void tma_box(uint32_t dst_smem, const CUtensorMap* tm
   asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst_smem),
                "l"(reinterpret_cast<uint64_t>(tm)), "r"(col), "r"(row), "r"(bar)
                : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ double2 lds_f64x2(uint32_t a) {
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+  return v;
 }
 __device__ __forceinline__ double lds_f64(uint32_t a) {
   double v;
@@ -385,6 +396,12 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
   const uint32_t pool_s = (uint32_t)__cvta_generic_to_shared(pool);
   const uint32_t x_s = pool_s + (uint32_t)((kPoolDoubles + CT * TLD) * sizeof(double));
   const uint32_t bar_s = pool_s + (uint32_t)((kPoolDoubles + 2 * CT * TLD + CT) * sizeof(double));   // full[NST], empty[NST]
+  // chain CTA: compute warps -> publisher warp: R_inv (L_jj and W_jj are in shared memory), R_trsm (the stores of L(j+1,j)
+  // are issued); publisher -> compute warps: F_x (X has been read: the next inverse may overwrite it), F_d (the diagonal
+  // buffer has been read: the next TRSM may overwrite it)
+  const uint32_t rel_s = bar_s + 8u * (2 * NST);
+  const uint32_t R_inv = rel_s, R_trsm = rel_s + 8u, F_x = rel_s + 16u, F_d = rel_s + 24u;
+  double* T2 = pool + kChainStages * kStageBytes / 8;   // chain CTA: third 64 x TLD tile buffer, in the unused half of the ring
   int* fL = flags;
   int* fB = flags + (size_t)nt * nt;
   int* fP = fB + (size_t)nt * nt;
@@ -393,17 +410,95 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       cmbar_init(bar_s + 8u * q, 1);                       // full: the producer's arrive.expect_tx (+ the bytes)
       cmbar_init(bar_s + 8u * (NST + q), kCholWarps);      // empty: one arrival per compute warp
     }
+    cmbar_init(R_inv, kCholWarps); cmbar_init(R_trsm, kCholWarps); cmbar_init(F_x, 1); cmbar_init(F_d, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();                                         // the only CTA-wide barrier: the producer warp leaves here
   const int t_beg = list_off[blockIdx.x], t_end = list_off[blockIdx.x + 1];
 
   if (tid >= kCholThreads) {
-    // ---- producer warp: for every k-loop of this CTA's list, in order: wait for the operands' flags (the lanes look at
+    // ---- producer warp (and, in the chain CTA, the publisher warp).  Producer: for every k-loop of this CTA's list, in order: wait for the operands' flags (the lanes look at
     // up to 32 k-tiles at once), wait for a free stage, and stream the two 64 x 32 operand chunks into it: four 2-D TMA
     // boxes (cp.async.bulk.tensor, 128-byte swizzle), issued by one lane.
     const int lane = tid & 31;
     uint32_t st = 0, ph = 0;
+    const bool chain_cta = t_beg < t_end && tasks[t_beg].type >= 2;   // its list then holds chain tasks only
+    if (tid >= kCholThreads + 32) {
+      // ---- publisher warp (chain CTA only): writes the chain's results to global memory and publishes them, so that the
+      // compute warps go straight from the inverse to TRSM.  Per column j: W_jj (from X) -> flag fL[j][j] (the column's tiles
+      // wait for it: it goes first), Wt_jj -> flag fB[j][j], L_jj (and Lt_jj) from the diagonal buffer; then the flag of
+      // L(j+1,j), whose stores the compute warps issue themselves (the st.release fence waits for them here, not there).
+      if (!chain_cta) return;
+      const double* D = S;
+      const double* O = T2;
+      uint32_t p_inv = 0, p_trsm = 0;
+      for (int ti = t_beg; ti < t_end; ++ti) {
+        const CholTask tk = tasks[ti];
+        const int j_ = tk.j;
+        if (tk.type == 2) {
+          cmbar_wait(R_inv, p_inv); p_inv ^= 1u;
+          const size_t g0 = (size_t)(j_ * CT) * P + j_ * CT;
+#pragma unroll 8
+          for (int r = 0; r < CT; ++r)
+            *reinterpret_cast<double2*>(W + g0 + (size_t)r * P + 2 * lane) = *reinterpret_cast<const double2*>(X + r * TLD + 2 * lane);
+          __syncwarp();
+          if (lane == 0) st_release(&fL[(size_t)j_ * nt + j_], 1);
+          // transposes: 8 rows x 4 columns per step in the pattern of a DMMA fragment (conflict-free with the padded
+          // stride), 8 lanes store 64 contiguous bytes of a transposed row
+          const int g = lane >> 2, t = lane & 3;
+#pragma unroll 8
+          for (int b = 0; b < (CT / 8) * (CT / 4); ++b) {
+            const int r = (b / (CT / 4)) * 8 + g, c = (b % (CT / 4)) * 4 + t;
+            Wt[g0 + (size_t)c * P + r] = X[r * TLD + c];
+          }
+          __syncwarp();
+          if (lane == 0) { st_release(&fB[(size_t)j_ * nt + j_], 1); cmbar_arrive(F_x); }
+#pragma unroll 8
+          for (int r = 0; r < CT; ++r) {
+            const int c = 2 * lane;
+            double2 l = *reinterpret_cast<const double2*>(D + r * TLD + c);
+            if (c > r) l.x = 0.0;
+            if (c + 1 > r) l.y = 0.0;
+            *reinterpret_cast<double2*>(L + g0 + (size_t)r * P + c) = l;
+          }
+          if (Lt != nullptr) {   // L^T, used by the block back-substitution when only a block-diagonal inverse is built
+#pragma unroll 8
+            for (int b = 0; b < (CT / 8) * (CT / 4); ++b) {
+              const int r = (b / (CT / 4)) * 8 + g, c = (b % (CT / 4)) * 4 + t;
+              Lt[g0 + (size_t)c * P + r] = c <= r ? D[r * TLD + c] : 0.0;
+            }
+          }
+          __syncwarp();
+          if (j_ + 1 < nt) {                                   // the flag of L(j+1,j): its stores were issued by TRSM(j)
+            cmbar_wait(R_trsm, p_trsm); p_trsm ^= 1u;
+            if (lane == 0) st_release(&fL[(size_t)(j_ + 1) * nt + j_], 1);
+          }
+          // F_d last: a phase of any of these barriers completes only after the other side has consumed the previous one
+          // (parity waits cannot tell phases two apart)
+          if (lane == 0) cmbar_arrive(F_d);
+          { const double* q = D; D = O; O = q; }               // the buffers swap roles every column
+        }
+      }
+      return;
+    }
+    if (chain_cta) {
+      // ---- producer warp of the chain CTA: lane 0 fetches the parked accumulators of TRSM / SYRK (32 KB, contiguous) into
+      // ring stages as soon as their prefix tasks have stored them -- normally while POTRF is still running
+      if (lane == 0) {
+        for (int ti = t_beg; ti < t_end; ++ti) {
+          const CholTask tk = tasks[ti];
+          if (tk.type < 3 || tk.slot_in < 0) continue;
+          const uint32_t full = bar_s + 8u * st, empty = bar_s + 8u * (NST + st);
+          while (ld_acquire(&fP[tk.slot_in]) == 0) __nanosleep(20);
+          asm volatile("fence.proxy.async.global;" ::: "memory");
+          cmbar_wait(empty, ph ^ 1u);
+          cmbar_expect_tx(full, (uint32_t)(CT * CT * sizeof(double)));
+          bulk_g2s(pool_s + st * (uint32_t)kStageBytes, ws + (size_t)tk.slot_in * CT * CT, (uint32_t)(CT * CT * sizeof(double)), full);
+          if (++st == kChainStages) { st = 0; ph ^= 1u; }
+        }
+      }
+      return;
+    }
     for (int ti = t_beg; ti < t_end; ++ti) {
       const CholTask tk = tasks[ti];
       if (tk.type >= 2 || tk.kend <= tk.kbeg) continue;
@@ -420,7 +515,7 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
             if (kq < tk.kend) {
               ok = ld_acquire(&fL[(size_t)ra * nt + kq]) != 0;
               if (isL) { if (rb != ra) ok = (ld_acquire(&fL[(size_t)rb * nt + kq]) != 0) && ok; }
-              else ok = (ld_acquire(kq == rb ? &fL[(size_t)rb * nt + rb] : &fB[(size_t)rb * nt + kq]) != 0) && ok;
+              else ok = (ld_acquire(&fB[(size_t)rb * nt + kq]) != 0) && ok;   // kq == rb: the diagonal tile Wt_ii
             }
             const unsigned m = __ballot_sync(0xffffffffu, ok);
             n = __ffs(~m) - 1;
@@ -484,6 +579,19 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       a[q >> 1][q & 1][0] = v.x; a[q >> 1][q & 1][1] = v.y;
     }
   };
+  // the same accumulator, prefetched into the next ring stage by the producer warp (chain tasks)
+  auto load_slot_ring = [&](double (&a)[kMB][2][2]) {
+    cmbar_wait(bar_s + 8u * c_st, c_ph);
+    const uint32_t src = pool_s + c_st * (uint32_t)kStageBytes + (uint32_t)(tid * sizeof(double2));
+#pragma unroll
+    for (int q = 0; q < 2 * kMB; ++q) {
+      const double2 v = lds_f64x2(src + (uint32_t)(q * kCholThreads * sizeof(double2)));
+      a[q >> 1][q & 1][0] = v.x; a[q >> 1][q & 1][1] = v.y;
+    }
+    __syncwarp();
+    if ((tid & 31) == 0) cmbar_arrive(bar_s + 8u * (NST + c_st));
+    if (++c_st == kChainStages) { c_st = 0; c_ph ^= 1u; }
+  };
   auto acc_to_smem = [&](const double (&a)[kMB][2][2], double* T) {
 #pragma unroll
     for (int mb = 0; mb < kMB; ++mb)
@@ -491,7 +599,9 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       for (int nb = 0; nb < 2; ++nb)
         *reinterpret_cast<double2*>(T + (f.row0 + mb * 8 + f.g) * TLD + f.col0 + nb * 8 + 2 * f.t) = make_double2(a[mb][nb][0], a[mb][nb][1]);
   };
-  // diagonal tile: L_jj = chol(S), W_jj = L_jj^-1 (X), both written out (with Wt and, if asked for, Lt); flag released
+  // diagonal tile outside the chain CTA (single-CTA schedules): L_jj = chol(S), W_jj = L_jj^-1 (X), both written out (with Wt
+  // and, if asked for, Lt).  W_jj is published by flag fL[j][j] (the off-diagonal tiles of the column wait for it), Wt_jj by
+  // fB[j][j] (inverse tiles).
   auto diag_finish = [&](int j_) {
     const bool ok = tile_potrf(S, rdiag, tid);
     if (!ok && tid == 0) atomicCAS(&ctl->status, 0, -4);
@@ -499,18 +609,27 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
     for (int e = tid; e < CT * CT / 2; e += kCholThreads) {
       const int r = e / (CT / 2), c = (e % (CT / 2)) * 2;
       const size_t g = (size_t)(j_ * CT + r) * P + j_ * CT + c;
+      *reinterpret_cast<double2*>(W + g) = *reinterpret_cast<const double2*>(X + r * TLD + c);
       double2 l = *reinterpret_cast<const double2*>(S + r * TLD + c);
       if (c > r) l.x = 0.0;
       if (c + 1 > r) l.y = 0.0;
       *reinterpret_cast<double2*>(L + g) = l;
-      *reinterpret_cast<double2*>(W + g) = *reinterpret_cast<const double2*>(X + r * TLD + c);
-      *reinterpret_cast<double2*>(Wt + g) = make_double2(X[c * TLD + r], X[(c + 1) * TLD + r]);
-      if (Lt != nullptr)   // L^T, used by the block back-substitution when only a block-diagonal inverse is built
-        *reinterpret_cast<double2*>(Lt + g) = make_double2(c >= r ? S[c * TLD + r] : 0.0, c + 1 >= r ? S[(c + 1) * TLD + r] : 0.0);
+    }
+    {
+      const int g = (tid >> 2) & 7, t = tid & 3, w = tid >> 5;
+#pragma unroll 4
+      for (int b = w; b < (CT / 8) * (CT / 4); b += kCholWarps) {
+        const int r = (b / (CT / 4)) * 8 + g, c = (b % (CT / 4)) * 4 + t;
+        const size_t gt = (size_t)(j_ * CT + c) * P + j_ * CT + r;
+        Wt[gt] = X[r * TLD + c];
+        if (Lt != nullptr) Lt[gt] = c <= r ? S[r * TLD + c] : 0.0;
+      }
     }
     cta_sync();
-    if (tid == 0) st_release(&fL[(size_t)j_ * nt + j_], 1);
+    if (tid == 0) { st_release(&fL[(size_t)j_ * nt + j_], 1); st_release(&fB[(size_t)j_ * nt + j_], 1); }
   };
+  double* Dbuf = S;                                        // chain CTA: the diagonal tile being factored ...
+  double* Obuf = T2;                                       // ... and the sub-diagonal tile; they swap every column
 
   for (int ti = t_beg; ti < t_end; ++ti) {
     const CholTask tk = tasks[ti];
@@ -520,45 +639,66 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
       const int j = tk.j;
       double acc[kMB][2][2];
       if (tk.type == 2) {
-        // POTRF(j): S holds A_jj (left there by SYRK(j-1); column 0: the Q tile)
-        if (j == 0) { load_q_tile(0, 0, acc); acc_to_smem(acc, S); }
+        // POTRF(j): Dbuf holds A_jj (left there by SYRK(j-1); column 0: the Q tile).  The publisher warp writes the results out.
+        if (j == 0) { load_q_tile(0, 0, acc); acc_to_smem(acc, Dbuf); }
         cta_sync();
-        diag_finish(j);
+        const bool ok = tile_potrf(Dbuf, rdiag, tid);
+        if (!ok && tid == 0) atomicCAS(&ctl->status, 0, -4);
+        if (trace != nullptr && tid == 0) trace[4 * (size_t)ti + 1] = globaltimer_ns();
+        if (j > 0) {   // the publisher is done with column j-1: X may be overwritten, and so may the old diagonal buffer (TRSM(j))
+          cmbar_wait(F_x, (uint32_t)((j - 1) & 1));
+          cmbar_wait(F_d, (uint32_t)((j - 1) & 1));
+        }
+        tile_trinv(Dbuf, rdiag, X, tid);                        // ends with a barrier of the compute warps
+        if ((tid & 31) == 0) cmbar_arrive(R_inv);
+        if (trace != nullptr && tid == 0) trace[4 * (size_t)ti + 2] = globaltimer_ns();
       } else if (tk.type == 3) {
         // TRSM(j): L(j+1,j) = A W_jj^T, A = parked accumulator of (j+1,j) with every k < j applied (column 0: Q tile);
-        // W_jj is still in X.  The product goes to global memory and stays in S as the operand of SYRK(j).
-        if (tk.slot_in >= 0) load_slot(tk.slot_in, acc); else load_q_tile(j + 1, j, acc);
-        cta_sync();                              // everyone is done with S (L_jj was written out by POTRF(j))
-        acc_to_smem(acc, S);
+        // W_jj is still in X.  The product goes to global memory and stays in Obuf as the operand of SYRK(j).
+        if (tk.slot_in >= 0) load_slot_ring(acc); else load_q_tile(j + 1, j, acc);
+        // (Obuf was the diagonal buffer of column j-1: POTRF(j) has waited for the publisher to be done with it)
+        acc_to_smem(acc, Obuf);
         cta_sync();
         double out[kMB][2][2];
 #pragma unroll
         for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb) out[mb][nb][0] = out[mb][nb][1] = 0.0;
-        tile_mma<TLD, TLD, CT, false>(S, X, f, out);
+        tile_mma<TLD, TLD, CT, false>(Obuf, X, f, out);
 #pragma unroll
         for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb) {
             const int r = (j + 1) * CT + f.row0 + mb * 8 + f.g, c = j * CT + f.col0 + nb * 8 + 2 * f.t;
             *reinterpret_cast<double2*>(L + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
-            if (Lt != nullptr) { Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1]; }
           }
-        cta_sync();                              // the product has been read from S by every warp
-        acc_to_smem(out, S);
+        __syncwarp();
+        if ((tid & 31) == 0) cmbar_arrive(R_trsm);       // L(j+1,j) is on its way: the publisher warp sets its flag
+        if (Lt != nullptr) {
+#pragma unroll
+          for (int mb = 0; mb < kMB; ++mb)
+#pragma unroll
+            for (int nb = 0; nb < 2; ++nb) {
+              const int r = (j + 1) * CT + f.row0 + mb * 8 + f.g, c = j * CT + f.col0 + nb * 8 + 2 * f.t;
+              Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1];
+            }
+        }
+        cta_sync();                              // the product has been read from Obuf by every warp
+        acc_to_smem(out, Obuf);
         cta_sync();
-        if (tid == 0) st_release(&fL[(size_t)(j + 1) * nt + j], 1);
       } else {
-        // SYRK(j): A(j+1,j+1) = parked accumulator (every k < j applied; column 1: Q tile) - L(j+1,j) L(j+1,j)^T -> S
-        if (tk.slot_in >= 0) load_slot(tk.slot_in, acc); else load_q_tile(j + 1, j + 1, acc);
-        tile_mma<TLD, TLD, CT, true>(S, S, f, acc);
+        // SYRK(j): A(j+1,j+1) = parked accumulator (every k < j applied; column 1: Q tile) - L(j+1,j) L(j+1,j)^T -> Obuf,
+        // which becomes the diagonal buffer of column j+1
+        if (tk.slot_in >= 0) load_slot_ring(acc); else load_q_tile(j + 1, j + 1, acc);
+        tile_mma<TLD, TLD, CT, true>(Obuf, Obuf, f, acc);
         cta_sync();
-        acc_to_smem(acc, S);
+        acc_to_smem(acc, Obuf);
+        { double* q = Dbuf; Dbuf = Obuf; Obuf = q; }
       }
       if (trace != nullptr && tid == 0) {
         const unsigned long long tn = globaltimer_ns();
-        trace[4 * (size_t)ti + 1] = tn; trace[4 * (size_t)ti + 2] = tn; trace[4 * (size_t)ti + 3] = blockIdx.x;
+        if (tk.type != 2) { trace[4 * (size_t)ti + 1] = tn; trace[4 * (size_t)ti + 2] = tn; }
+        trace[4 * (size_t)ti + 3] = tn;                    // chain tasks (always CTA 0): the end time goes to the last word
       }
       continue;
     }
@@ -892,14 +1032,14 @@ cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_e
       // A large branch (p >= ~2000) that is longer than the pass: split the SMs so that both finish together.  The pass
       // streams X at full HBM bandwidth on ~kPassSatSms SMs and slows down in proportion below that; the branch is
       // bound by its work on few SMs and by the chain of diagonal tiles on many.  A split that does not beat running
-      // the two one after the other on every SM by 10 % is not taken.
+      // the two one after the other on every SM by 5 % is not taken.
       if (!found && nt > 20) {
-        double split_t = 0.9 * best_t;
-        for (int k : {64, 80, 96, 104, 112, 120, 128}) {
+        double split_t = 0.95 * best_t;
+        for (int k : {64, 72, 80, 88, 96, 104, 112, 120}) {
           if (k > tile_tasks || k > num_sms - 16) break;
           CholSchedule s = chol_build_schedule(nt, sb, k);
           const double pass_us = fused_us * std::max(1.0, kPassSatSms / (double)(num_sms - k));
-          const double t = std::max(pass_us, 1.15 * s.makespan_us);   // 1.15: tile loads compete with the X stream
+          const double t = std::max(pass_us, 1.05 * s.makespan_us);   // 1.05: tile loads compete with the X stream in L2
           if (t < split_t) { split_t = t; best = std::move(s); found = true; }
         }
       }

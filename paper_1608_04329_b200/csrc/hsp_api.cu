@@ -753,6 +753,10 @@ long long hsp_dbg_chol_trace(const hsp_state* s, long long* rows, long long capa
     r[0] = t.type; r[1] = t.i; r[2] = t.j; r[3] = t.kbeg; r[4] = t.kend; r[5] = t.slot_in; r[6] = t.slot_out;
     r[7] = (long long)tr[4 * q + 3]; r[8] = (long long)tr[4 * q]; r[9] = (long long)tr[4 * q + 1]; r[10] = (long long)tr[4 * q + 2];
     r[11] = 0;
+    if (t.type >= 2) {   // chain tasks run on CTA 0; the device keeps their end time in the last trace word
+      r[7] = 0; r[10] = (long long)tr[4 * q + 3];
+      if (t.type == 2) r[11] = (long long)tr[4 * q + 2];   // POTRF: r[9] = end of the tile factorisation, r[11] = end of the inverse
+    }
   }
   return n;
 }
