@@ -156,18 +156,23 @@ struct Frag {
 };
 
 // acc[m][n] += sgn * sum_k A[m][k] B[n][k],  k in [0, K): A and B are row-major [row][k] in shared memory.
-template <int LDA, int LDB, int K, bool NEG>
+// PERM: a DMMA multiplies the k-columns {2m, 2m+1, 8+2m, 9+2m} of each group of 16 (the grouping of the k-loops,
+// tile_mma_s) instead of four consecutive ones -- used where a chain task replaces a k-loop step (SYRK), so that the
+// rounding, and with it every bit of L, does not depend on the number of CTAs.
+template <int LDA, int LDB, int K, bool NEG, bool PERM = false>
 __device__ __forceinline__ void tile_mma(const double* __restrict__ A, const double* __restrict__ B, const Frag& f,
                                          double (&acc)[kMB][2][2]) {
-  const double* ap = A + (f.row0 + f.g) * LDA + f.t;
-  const double* bp = B + (f.col0 + f.g) * LDB + f.t;
+  const int tk = PERM ? (f.t >> 1) * 8 + (f.t & 1) : f.t;
+  const double* ap = A + (f.row0 + f.g) * LDA + tk;
+  const double* bp = B + (f.col0 + f.g) * LDB + tk;
 #pragma unroll
   for (int kk = 0; kk < K; kk += 4) {
+    const int ko = PERM ? (kk / 16) * 16 + ((kk % 16) / 4) * 2 : kk;
     double a[kMB], b[2];
 #pragma unroll
-    for (int mb = 0; mb < kMB; ++mb) { a[mb] = ap[mb * 8 * LDA + kk]; if (NEG) a[mb] = -a[mb]; }
+    for (int mb = 0; mb < kMB; ++mb) { a[mb] = ap[mb * 8 * LDA + ko]; if (NEG) a[mb] = -a[mb]; }
 #pragma unroll
-    for (int nb = 0; nb < 2; ++nb) b[nb] = bp[nb * 8 * LDB + kk];
+    for (int nb = 0; nb < 2; ++nb) b[nb] = bp[nb * 8 * LDB + ko];
 #pragma unroll
     for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
@@ -177,16 +182,19 @@ __device__ __forceinline__ void tile_mma(const double* __restrict__ A, const dou
 
 // The k-loop version: operands are TMA boxes in shared memory (32-bit shared-window addresses A, B: KC / 16 boxes each, a
 // box = 64 rows x 128 bytes with the 128-byte swizzle: the 16-byte unit u of row r sits at unit u ^ (r & 7)).  A lane
-// reads element (row0 + 8 mb + g, kk + t): its row has r & 7 = g whatever mb, so the four swizzled offsets of a box
-// (kk mod 16 = 0, 4, 8, 12) are per-lane constants `sw`.  The 32 lanes of an LDS.64 touch every 16-byte bank group exactly twice
-// (rows g and g ^ 1): two wavefronts for 256 bytes, i.e. conflict-free.
+// reads row (row0 + 8 mb + g), whose r & 7 = g whatever mb, so its swizzled offsets inside a box are per-lane constants.
+// Which four k-columns a DMMA multiplies is free (the same choice for A and B): step m = 0..3 of a box takes
+// k = {2m, 2m+1, 8+2m, 9+2m} for t = 0..3, i.e. unit ((t >> 1) * 4 + m) ^ g, half t & 1.  The 16 lanes of a half-warp
+// (g = 0..3 or 4..7) then touch 16 different (unit, half) pairs = all 32 banks once: two wavefronts per LDS.64, the
+// minimum.  (Consecutive k = 4m + t put rows g and g ^ 1 on the same unit: a 2-way conflict, measured as 2x the ideal
+// wavefronts on every fragment load.)
 struct SwzFrag {
   uint32_t a0, b0, sw[4];
   __device__ __forceinline__ explicit SwzFrag(const Frag& f) {
     a0 = (uint32_t)((f.row0 + f.g) * 128);
     b0 = (uint32_t)((f.col0 + f.g) * 128);
 #pragma unroll
-    for (int q = 0; q < 4; ++q) sw[q] = (uint32_t)((((2 * q + (f.t >> 1)) ^ f.g) * 16) + (f.t & 1) * 8);
+    for (int q = 0; q < 4; ++q) sw[q] = (uint32_t)(((((f.t >> 1) * 4 + q) ^ f.g) * 16) + (f.t & 1) * 8);
   }
 };
 template <bool NEG>
@@ -690,7 +698,7 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
         // SYRK(j): A(j+1,j+1) = parked accumulator (every k < j applied; column 1: Q tile) - L(j+1,j) L(j+1,j)^T -> Obuf,
         // which becomes the diagonal buffer of column j+1
         if (tk.slot_in >= 0) load_slot_ring(acc); else load_q_tile(j + 1, j + 1, acc);
-        tile_mma<TLD, TLD, CT, true>(Obuf, Obuf, f, acc);
+        tile_mma<TLD, TLD, CT, true, true>(Obuf, Obuf, f, acc);
         cta_sync();
         acc_to_smem(acc, Obuf);
         { double* q = Dbuf; Dbuf = Obuf; Obuf = q; }

@@ -293,3 +293,24 @@ def test_narrow_kernel_fused_pass_only(name, n_rows, p, U, shift, eta_mode, hsp_
     f32 = wl.X.dtype == torch.float32
     assert ez < ((2e-6 if eta_mode else 1e-9) if f32 else 1e-11) and eg < (1e-5 if f32 else 1e-11)
     g.close()
+
+
+def test_cholesky_does_not_depend_on_the_number_of_ctas(hsp_options):
+    """every tile is accumulated in ascending k by a fixed sequence of products, whatever the schedule --
+    one CTA (prefix + finish tasks), a chain CTA plus a few or many others: L and the draws are bit-identical.  (The grid
+    of the fused pass is pinned: the per-CTA partials of X^T z are fp32 chains, whose grouping follows the grid.)"""
+    wl = hsp_synth.make("C3", "cuda", n_rows=3001, p=640)         # nt = 10 tile rows
+    ref = None
+    hsp_options("fused_grid", 64)
+    for K in (1, 2, 3, 7, 20):
+        hsp_options("chol_ctas", K)
+        g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+        assert g.plan()["chol_ctas"] == K
+        g.sweep(3)
+        out = (g.get_chol(), *g.get_draws())
+        g.close()
+        if ref is None:
+            ref = out
+        else:
+            for a, b in zip(out, ref):
+                assert np.array_equal(a, b), K
