@@ -246,6 +246,7 @@ def main():
     ap.add_argument("--graph", action="store_true", help="replay the captured CUDA graph in the timed region (no per-kernel events)")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="plan-time option of libhsp.so (hsp_set_option), e.g. chol_ctas=24")
     ap.add_argument("--create-only", action="store_true", help="time hsp_create (device-resident X; Gram included) --steps times and exit")
+    ap.add_argument("--chol-trace", action="store_true", help="per-task device timestamps of the Cholesky task graph (option chol_trace) on a row sample of the workload; prints a summary and exits")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -280,6 +281,34 @@ def main():
     wl = hsp_synth.make(args.workload, dev)
     seed = multi.chain_seed(wl.seed, rank)
     stream = torch.cuda.Stream(device=dev)
+
+    if args.chol_trace:
+        # rows c, d1 alone: per-task timestamps of chol_task_kernel (hsp_dbg_chol_trace) over three direct-launch sweeps
+        hsp.set_option("chol_trace", 1)
+        wls = hsp_synth.make(args.workload, dev, n_rows=min(wl.N, 8009))
+        c = hsp.HorseshoeProbit(wls.X, wls.y, seed)
+        c.set_flags(hsp.HSP_NO_GRAPH | hsp.HSP_SERIAL)
+        c.sweep(3); c.sync()
+        tr = c.chol_trace()
+        typ, ke, kb, ts, tk, te = tr[:, 0], tr[:, 4], tr[:, 3], tr[:, 8], tr[:, 9], tr[:, 10]
+        out = {"metric": "chol_task_trace", "config": {"workload": WORKLOAD_DESC[args.workload], "p": wl.p, "plan": c.plan()},
+               "tasks": int(len(tr)), "makespan_us": float(te.max() - ts.min()) / 1e3, "by_type_mean_us": {}}
+        names = {0: "tile L(i,j)", 1: "inverse tile", 2: "POTRF (chain)", 3: "TRSM (chain)", 4: "SYRK (chain)"}
+        for t in sorted(set(typ.tolist())):
+            m = typ == t
+            out["by_type_mean_us"][names[t]] = {"n": int(m.sum()), "mean": float((te[m] - ts[m]).mean()) / 1e3}
+        m = (typ == 0) & (ke - kb >= 4)
+        if m.any():
+            out["kloop_us_per_64x64x64_product"] = {"median": float(np.median((tk[m] - ts[m]) / 1e3 / (ke[m] - kb[m]))),
+                                                    "p10": float(np.percentile((tk[m] - ts[m]) / 1e3 / (ke[m] - kb[m]), 10))}
+        m2 = typ == 2
+        if m2.any():
+            po = np.sort(ts[m2])
+            out["chain"] = {"potrf_us": float((tk[m2] - ts[m2]).mean()) / 1e3, "inverse_us": float((tr[:, 11][m2] - tk[m2]).mean()) / 1e3,
+                            "period_us_per_column": float(np.median(np.diff(po))) / 1e3 if len(po) > 1 else None}
+        c.close()
+        print(json.dumps(out), flush=True)
+        return
 
     if args.create_only:
         times = []
