@@ -180,6 +180,44 @@ __device__ __forceinline__ void tile_mma(const double* __restrict__ A, const dou
   }
 }
 
+// out[m][n] += sum_{k <= n} A[m][k] Wm[n][k] for a LOWER-TRIANGULAR Wm (the product A W_jj^T that finishes an off-diagonal
+// tile): the 8-column block cb needs only k < 8 (cb + 1).  A warp takes the column blocks {wc, 7 - wc} (wc = warp / 2) of
+// its 32 rows, i.e. 72 of the 128 k-steps of the full product whatever wc -- balanced.  acc[mb][nb] is the block
+// (row0 / 8 + mb, nb == 0 ? wc : 7 - wc); the skipped terms are exact zeros.
+struct TriFrag {
+  int row0, g, t, cb[2];
+  __device__ __forceinline__ explicit TriFrag(int tid) {
+    const int w = tid >> 5, lane = tid & 31;
+    row0 = (w & 1) * 32; g = lane >> 2; t = lane & 3; cb[0] = w >> 1; cb[1] = 7 - (w >> 1);
+  }
+  __device__ __forceinline__ int col(int nb) const { return cb[nb] * 8 + 2 * t; }   // first of the two columns of acc[.][nb]
+};
+template <int LDA, int LDB>
+__device__ __forceinline__ void tile_mma_tri(const double* __restrict__ A, const double* __restrict__ Wm, const TriFrag& z,
+                                             double (&acc)[kMB][2][2]) {
+  static_assert(kMB == 4, "the triangular product assumes 32 x 16 warp tiles");
+  const double* ap = A + (z.row0 + z.g) * LDA + z.t;
+  const double* b0 = Wm + (z.cb[0] * 8 + z.g) * LDB + z.t;
+  const double* b1 = Wm + (z.cb[1] * 8 + z.g) * LDB + z.t;
+  const int lim0 = 8 * (z.cb[0] + 1), lim1 = 8 * (z.cb[1] + 1);      // lim0 <= 32 < lim1, warp-uniform
+#pragma unroll
+  for (int kk = 0; kk < CT; kk += 4) {
+    if (kk < lim1) {
+      double a[kMB];
+#pragma unroll
+      for (int mb = 0; mb < kMB; ++mb) a[mb] = ap[mb * 8 * LDA + kk];
+      const double bb1 = b1[kk];
+#pragma unroll
+      for (int mb = 0; mb < kMB; ++mb) dmma(acc[mb][1], a[mb], bb1);
+      if (kk < lim0) {
+        const double bb0 = b0[kk];
+#pragma unroll
+        for (int mb = 0; mb < kMB; ++mb) dmma(acc[mb][0], a[mb], bb0);
+      }
+    }
+  }
+}
+
 // The k-loop version: operands are TMA boxes in shared memory (32-bit shared-window addresses A, B: KC / 16 boxes each, a
 // box = 64 rows x 128 bytes with the 128-byte swizzle: the 16-byte unit u of row r sits at unit u ^ (r & 7)).  A lane
 // reads row (row0 + 8 mb + g), whose r & 7 = g whatever mb, so its swizzled offsets inside a box are per-lane constants.
@@ -558,6 +596,7 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
 
   const Frag f(tid);
   const SwzFrag zf(f);
+  const TriFrag zt(tid);
   uint32_t c_st = 0, c_ph = 0;                             // the compute warps' position in the ring
   const double tau_inv2 = ctl->tau_inv2;
 
@@ -672,12 +711,12 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
         for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb) out[mb][nb][0] = out[mb][nb][1] = 0.0;
-        tile_mma<TLD, TLD, CT, false>(Obuf, X, f, out);
+        tile_mma_tri<TLD, TLD>(Obuf, X, zt, out);
 #pragma unroll
         for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb) {
-            const int r = (j + 1) * CT + f.row0 + mb * 8 + f.g, c = j * CT + f.col0 + nb * 8 + 2 * f.t;
+            const int r = (j + 1) * CT + zt.row0 + mb * 8 + zt.g, c = j * CT + zt.col(nb);
             *reinterpret_cast<double2*>(L + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
           }
         __syncwarp();
@@ -687,12 +726,16 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
           for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb) {
-              const int r = (j + 1) * CT + f.row0 + mb * 8 + f.g, c = j * CT + f.col0 + nb * 8 + 2 * f.t;
+              const int r = (j + 1) * CT + zt.row0 + mb * 8 + zt.g, c = j * CT + zt.col(nb);
               Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1];
             }
         }
         cta_sync();                              // the product has been read from Obuf by every warp
-        acc_to_smem(out, Obuf);
+#pragma unroll
+        for (int mb = 0; mb < kMB; ++mb)
+#pragma unroll
+          for (int nb = 0; nb < 2; ++nb)
+            *reinterpret_cast<double2*>(Obuf + (zt.row0 + mb * 8 + zt.g) * TLD + zt.col(nb)) = make_double2(out[mb][nb][0], out[mb][nb][1]);
         cta_sync();
       } else {
         // SYRK(j): A(j+1,j+1) = parked accumulator (every k < j applied; column 1: Q tile) - L(j+1,j) L(j+1,j)^T -> Obuf,
@@ -774,13 +817,13 @@ chol_task_kernel(const double* __restrict__ G, const double* __restrict__ lam_in
                 make_double2(acc[mb][nb][0], acc[mb][nb][1]);
         cp_async_wait<0>();
         cta_sync();
-        tile_mma<TLD, TLD, CT, false>(S, X, f, out);               // L_ij = A W_jj^T
+        tile_mma_tri<TLD, TLD>(S, X, zt, out);                     // L_ij = A W_jj^T
 #pragma unroll
         for (int mb = 0; mb < kMB; ++mb)
 #pragma unroll
           for (int nb = 0; nb < 2; ++nb)
           {
-            const int r = i * CT + f.row0 + mb * 8 + f.g, c = j * CT + f.col0 + nb * 8 + 2 * f.t;
+            const int r = i * CT + zt.row0 + mb * 8 + zt.g, c = j * CT + zt.col(nb);
             *reinterpret_cast<double2*>(L + (size_t)r * P + c) = make_double2(out[mb][nb][0], out[mb][nb][1]);
             if (Lt != nullptr) { Lt[(size_t)c * P + r] = out[mb][nb][0]; Lt[(size_t)(c + 1) * P + r] = out[mb][nb][1]; }
           }
