@@ -1089,7 +1089,7 @@ cudaError_t chol_plan_create(CholPlan* pl, int p, int num_sms, double fused_ms_e
         for (int k : {64, 72, 80, 88, 96, 104, 112, 120}) {
           if (k > tile_tasks || k > num_sms - 16) break;
           CholSchedule s = chol_build_schedule(nt, sb, k);
-          const double pass_us = fused_us * std::max(1.0, kPassSatSms / (double)(num_sms - k));
+          const double pass_us = fused_us * std::max(1.0, kPassSatSms / (double)(num_sms - k - 2));   // two SMs stay spare (hsp_api.cu)
           const double t = std::max(pass_us, 1.05 * s.makespan_us);   // 1.05: tile loads compete with the X stream in L2
           if (t < split_t) { split_t = t; best = std::move(s); found = true; }
         }

@@ -206,7 +206,14 @@ static int create_common(hsp_state** out, hsp_state* s) {
   const double fused_ms_est = x_bytes / 7.0e9 + 0.01;   // the pass streams X at ~7.2 TB/s on B200 (profiles/)
   { std::lock_guard<std::mutex> lock(g_opt_mutex); s->opt = g_default_options; }
   CK(chol_plan_create(&s->chol, p, s->num_sms, fused_ms_est, s->opt));
-  const int fused_sms = s->chol.overlap ? s->num_sms - s->chol.K : s->num_sms;
+  // Two SMs are left to neither: with every SM spoken for, a single SM that is busy for a moment when the Cholesky branch
+  // starts (any other kernel of the process, a driver-side copy kernel) leaves one of its CTAs without a home until the
+  // persistent pass ends -- and the tiles that CTA owns stall the whole task graph: the sweep then takes pass + branch
+  // instead of max(pass, branch).  Measured by forcing one CTA too many: C3 0.583 -> 0.878 ms, C4 1.52 -> 2.73 ms; the same
+  // signature showed up unforced in about one bench run in ten.  The pass is HBM-bound with SMs to spare (8.1): 130 instead
+  // of 132 CTAs cost < 1 %.
+  const int kSpareSms = 2;
+  const int fused_sms = s->chol.overlap ? std::max(1, s->num_sms - s->chol.K - kSpareSms) : s->num_sms;
   s->plan = fused_plan(s->dtype, N, p, fused_sms, s->X, s->opt);
   s->plan.row_offset = s->row_offset;
   // set opt-in shared-memory attributes now, outside any stream capture

@@ -80,7 +80,8 @@ cudaError_t gram_finish_launch(const GramPlan& g, int p, const double* scratch, 
 // One tile task of the Cholesky task graph (64x64 tiles).  type 0: tile L(i,j), i >= j; type 1: inverse tile
 // W(j,i), i < j.  The task accumulates k in [kbeg, kend); slot_in >= 0: start from the partial accumulator in
 // that workspace slot (else from the Q tile / zero); slot_out >= 0: store the partial accumulator there
-// instead of finalising the tile.
+// instead of finalising the tile.  Types 2, 3, 4: the chain tasks POTRF(j), TRSM(j) -> L(j+1,j), SYRK(j) -> A(j+1,j+1) of
+// the dedicated chain CTA (first list, schedules with K >= 2).
 struct CholTask { int type, i, j, kbeg, kend, slot_in, slot_out, pad; };
 struct CholSchedule {
   int K = 0, n_slots = 0;
@@ -100,7 +101,7 @@ struct CholPlan {
   int* d_flags = nullptr;            // [nt*nt] L tiles, [nt*nt] inverse tiles, [n_slots] partials
   size_t n_flags = 0;
   double* d_ws = nullptr;            // n_slots x 4096 doubles
-  unsigned long long* d_trace = nullptr;   // HSP_CHOL_TRACE=1: per task {start, k-loop end, end} ns and the CTA
+  unsigned long long* d_trace = nullptr;   // option chol_trace = 1: four words per task: start, end of the k-loop, end (ns), CTA (chain tasks: see hsp.h)
   std::vector<CholTask> h_tasks;     // host copy of the schedule (for hsp_dbg_chol_trace)
 };
 int chol_tiles(int p);                 // nt = ceil(p / 64)
