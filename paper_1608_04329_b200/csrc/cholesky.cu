@@ -23,10 +23,12 @@
 // accumulated in ascending k by a fixed sequence of tasks: the result does not depend on the number of CTAs.
 //
 // Tile products run on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> SASS DMMA; tcgen05 has no f64 kind):
-// 8 warps x (32 rows x 16 columns) of the 64x64 accumulator.  Operands are staged in 32-column chunks by a PRODUCER WARP
-// (cp.async.bulk, one 256-byte copy per tile row into a padded row stride that makes the fragment loads
-// conflict-free; 4-stage ring, full / empty mbarriers).  The producer also does all the flag polling for the k-loops and
-// runs ahead of the compute warps across tasks, so the next task's operands arrive during this task's epilogue.
+// 8 warps x (32 rows x 16 columns) of the 64x64 accumulator.  CTA = 8 compute warps + a PRODUCER warp + a PUBLISHER warp.
+// The producer streams the operands of the k-loops in 32-column chunks as 2-D TMA boxes (cp.async.bulk.tensor, 16 columns
+// x 64 rows with the 128-byte swizzle, which makes the fragment loads conflict-free without padding; 4-stage ring, full /
+// empty mbarriers), does all the flag polling for the k-loops and runs ahead of the compute warps across tasks, so the
+// next task's operands arrive during this task's epilogue.  In the chain CTA the producer fetches the parked accumulators
+// and the publisher warp writes the chain's results to global memory and sets their flags.
 //
 // Storage: row-major, leading dimension P; L lower, W lower, Wt upper.
 #include <cuda.h>
@@ -59,10 +61,6 @@ constexpr size_t kCholSmem = 1024 + (size_t)(kPoolDoubles + 2 * CT * TLD + CT) *
 int chol_tiles(int p) { return (p + CT - 1) / CT; }
 int chol_ld(int p) { return chol_tiles(p) * CT; }
 
-__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
-               : "memory");
-}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
