@@ -343,6 +343,9 @@ def main():
             chain = hsp.HorseshoeProbit(wl.X, wl.y, seed, stream=stream)
             chain.set_flags((0 if args.graph else hsp.HSP_NO_GRAPH) | (hsp.HSP_PAPER_DESIGN if args.paper_design else 0))
             run_sweeps = chain.sweep
+        # history capacity for the longest timed call, allocated now: growing it inside a timed region stalls the GPU
+        # behind cudaFree / cudaMalloc (occasionally 0.1 - 1 s on this pool: profiles/r02_d_final.md)
+        chain.reserve_history(max(args.steps, wl.n_sweeps))
         run_sweeps(args.warmup)
         k0 = chain.launch_count()
         ms, fused_ms, fused_n = timed_sweeps(chain, run_sweeps, args.steps, stream, dev, clocks, dist, world)

@@ -103,6 +103,10 @@ double* hsp_gram_device(hsp_state* s);  /* DEVICE, p*p doubles row-major (symmet
  * or non-finite state inside the sweeps is reported by the next synchronising call
  * (hsp_get_draws / hsp_get_state / hsp_sync) as HSP_ENOTPD / HSP_ENUMERIC.                       */
 int hsp_sweep(hsp_state* s, long long n_iter);
+/* Reserve device history for calls of up to n_iter sweeps (it only grows).  hsp_sweep grows it on demand, which
+ * synchronises the chain and allocates: a caller that times its sweeps, or must not allocate later, reserves first.
+ * The draws of the previous hsp_sweep call are discarded when the history grows.  Errors: HSP_EINVAL, HSP_ENOMEM.   */
+int hsp_reserve_history(hsp_state* s, long long n_iter);
 
 /* Copy the draws of the most recent hsp_sweep call: beta[n_iter*p],
  * lambda[n_iter*p], tau[n_iter], row-major by sweep.  ANY pointers; any may be NULL.

@@ -46,6 +46,7 @@ def lib():
     L.hsp_create.argtypes = [C.POINTER(vp), vp, C.c_int, vp, ll, C.c_int, ull, vp]
     L.hsp_create_host.argtypes = [C.POINTER(vp), vp, C.c_int, vp, ll, C.c_int, ull, vp]
     L.hsp_sweep.argtypes = [vp, ll]
+    L.hsp_reserve_history.argtypes = [vp, ll]
     L.hsp_create_shard.argtypes = [C.POINTER(vp), vp, C.c_int, vp, ll, C.c_int, ull, ll, vp]
     L.hsp_sweep_prepare.argtypes = [vp, ll]
     L.hsp_sweep_begin.argtypes = [vp]
@@ -164,6 +165,9 @@ class HorseshoeProbit:
     def sweep(self, n_iter):
         _check(lib().hsp_sweep(self._h, n_iter))
         self.n_last = n_iter
+
+    def reserve_history(self, n_iter):
+        _check(lib().hsp_reserve_history(self._h, n_iter))
 
     def sync(self):
         _check(lib().hsp_sync(self._h))

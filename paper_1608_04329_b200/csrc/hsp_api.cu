@@ -342,21 +342,28 @@ static int output_after_sweep(hsp_state* s, bool last_of_call) {
   return HSP_OK;
 }
 
-static int prepare_history(hsp_state* s, long long n_iter) {
+// Device history for at least n_iter sweeps.  Growing it synchronises the chain and calls cudaFree / cudaMalloc, which on
+// the boxes this was measured on occasionally takes 0.1 - 1 s (seen as a few per cent of hsp_sweep calls that "took twice as
+// long": the GPU sits idle meanwhile): callers that time sweeps reserve the capacity first (hsp_reserve_history).
+static int grow_history(hsp_state* s, long long n_iter) {
+  if (n_iter <= s->h_cap) return HSP_OK;
   const int p = s->p;
+  CK(cudaStreamSynchronize(s->stream));
+  if (s->stream3) CK(cudaStreamSynchronize(s->stream3));
+  if (s->h_beta) { cudaFree(s->h_beta); cudaFree(s->h_lambda); cudaFree(s->h_tau); s->h_beta = s->h_lambda = s->h_tau = nullptr; }
+  s->h_cap = 0; s->h_n = 0;
+  CK(cudaMalloc(&s->h_beta, (size_t)n_iter * p * sizeof(double)));
+  CK(cudaMalloc(&s->h_lambda, (size_t)n_iter * p * sizeof(double)));
+  CK(cudaMalloc(&s->h_tau, (size_t)n_iter * sizeof(double)));
+  s->h_cap = n_iter;
+  return HSP_OK;
+}
+
+static int prepare_history(hsp_state* s, long long n_iter) {
   // the copy stream may still be reading the history of the previous call: the new call's sweeps start after it
   if (s->o_last_done) CK(cudaStreamWaitEvent(s->stream, s->o_last_done, 0));
   s->o_pending_first = 0; s->o_pending = 0;
-  if (n_iter > s->h_cap) {
-    CK(cudaStreamSynchronize(s->stream));
-    if (s->stream3) CK(cudaStreamSynchronize(s->stream3));
-    if (s->h_beta) { cudaFree(s->h_beta); cudaFree(s->h_lambda); cudaFree(s->h_tau); s->h_beta = s->h_lambda = s->h_tau = nullptr; }
-    s->h_cap = 0;
-    CK(cudaMalloc(&s->h_beta, (size_t)n_iter * p * sizeof(double)));
-    CK(cudaMalloc(&s->h_lambda, (size_t)n_iter * p * sizeof(double)));
-    CK(cudaMalloc(&s->h_tau, (size_t)n_iter * sizeof(double)));
-    s->h_cap = n_iter;
-  }
+  { const int rc = grow_history(s, n_iter); if (rc != HSP_OK) return rc; }
   s->h_n = n_iter;
   if (n_iter == 0) return HSP_OK;
   // history window of this call: set by a one-thread kernel (its arguments are copied at launch: no host sync)
@@ -580,6 +587,14 @@ int hsp_set_flags(hsp_state* s, unsigned flags) {
   }
   s->flags = flags;
   return HSP_OK;
+}
+
+int hsp_reserve_history(hsp_state* s, long long n_iter) {
+  if (!s) return fail(HSP_EINVAL, "state is NULL");
+  if (n_iter < 0) return fail(HSP_EINVAL, "n_iter must be >= 0");
+  if (s->split_open) return fail(HSP_EINVAL, "hsp_reserve_history between hsp_sweep_begin and hsp_sweep_end");
+  if (s->split_left > 0 && n_iter > s->h_cap) return fail(HSP_EINVAL, "hsp_reserve_history inside a prepared run of sharded sweeps");
+  return grow_history(s, n_iter);
 }
 
 int hsp_sweep(hsp_state* s, long long n_iter) {

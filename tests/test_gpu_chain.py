@@ -225,3 +225,23 @@ def test_options_are_plan_time_and_process_wide(hsp_options):
     assert hsp.get_option("fused_variant") == -1
     # generic kernel (exact fp64 eta) vs the TMA kernel (fp32 chains): same chain within the fp32-X tolerance
     assert np.max(np.abs(b - b_ref)) < 1e-4 * max(1.0, np.max(np.abs(b_ref)))
+
+
+def test_reserve_history_changes_nothing_but_the_allocation_time():
+    """hsp_reserve_history: the same draws with and without it; a later, longer call still grows the history."""
+    wl = hsp_synth.make("C2", "cuda", n_rows=4000)
+    (b_ref, l_ref, t_ref), _ = _draws(wl, 9)
+    g = hsp.HorseshoeProbit(wl.X, wl.y, wl.seed)
+    g.reserve_history(64)
+    g.sweep(4)
+    g.reserve_history(8)                      # smaller than the capacity: nothing happens, the draws stay
+    b, l, t = g.get_draws()
+    assert np.array_equal(b, b_ref[:4]) and np.array_equal(t, t_ref[:4])
+    g.sweep(5)
+    b, l, t = g.get_draws()
+    assert np.array_equal(b, b_ref[4:]) and np.array_equal(l, l_ref[4:]) and np.array_equal(t, t_ref[4:])
+    g.sweep(100)                              # beyond the reservation: grows on demand
+    assert g.get_draws()[0].shape == (100, wl.p)
+    with pytest.raises(hsp.HspError):
+        g.reserve_history(-1)
+    g.close()
