@@ -184,6 +184,26 @@ const char* hsp_fused_variant(const hsp_state* s);
 int hsp_set_option(hsp_state* s, const char* key, long long value);
 int hsp_get_option(const hsp_state* s, const char* key, long long* value);
 
+/* Rows a1-a3 + b as ONE stateless call that ALLOCATES NOTHING (no cudaMalloc / cudaFree, no allocating library routine), for
+ * callers that cannot allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid it.  For a given
+ * beta and sweep number k it computes eta = X beta, z_i ~ TN(eta_i, 1) on the side fixed by y_i with the Philox
+ * counters (i, k, Z) of the chain, and g = X^T z -- the same kernels as hsp_sweep, the same
+ * values as a chain with that seed whose state is beta at sweep k.
+ *   X, y    DEVICE, as for hsp_create (y is NOT validated here: every byte must be 0 or 1)
+ *   beta    DEVICE p doubles (read);  g_out  DEVICE p doubles (written);  z_out  DEVICE N doubles or NULL
+ *   k       sweep number, 1 <= k < 2^32;  stream: cudaStream_t as void* (NULL = the legacy default stream)
+ * Scratch (per-CTA partials of X^T z, control block) lives in a static device array of hsp_noalloc_scratch_bytes() = 8 MiB +
+ * 256 B that every GPU which loads the library holds until the process exits.  Limit: (CTAs x row groups of the pass) x p <=
+ * 2^20 doubles -- on 148 SMs: p <= 7084 with the wide TMA kernel, any p <= 511 with the narrow one, p <= 1771 with the generic
+ * kernel (wide rows that are not a multiple of 16 bytes); larger problems get
+ * HSP_EINVAL (message: hsp_noalloc_last_error) and must use hsp_create / hsp_sweep.  All calls share the array: calls that
+ * overlap on the GPU (two streams, two host threads) RACE -- serialise them.  Asynchronous: returns after enqueueing.
+ * Errors: HSP_EINVAL, HSP_ECUDA.                                                                                       */
+int hsp_xtz_noalloc(const void* X, int x_dtype, const unsigned char* y, long long N, int p, unsigned long long seed,
+                    long long k, const double* beta, double* g_out, double* z_out, void* stream);
+long long hsp_noalloc_scratch_bytes(void);
+const char* hsp_noalloc_last_error(void);
+
 /* Device unit-test hooks (one thread per element; DEVICE pointers):
  *   philox : out[4n] = Philox-4x32-10(ctr[4n], key[2n])
  *   uniform: ua[n], ub[n] from (seed, idx[n], sweep, tag) -- the variate addressing of the sweep

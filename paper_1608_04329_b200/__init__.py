@@ -6,4 +6,5 @@ no CPU fallback: importing works anywhere, but every compute call needs the CUDA
 """
 from .binding import (HSP_F32, HSP_F64, HSP_STORE_Z, HSP_FREEZE_SCALES, HSP_FREEZE_Z, HSP_FREEZE_BETA,  # noqa: F401
                       HSP_NO_GRAPH, HSP_SERIAL, HSP_PAPER_DESIGN, HspError, HorseshoeProbit, lib, lib_path, declared_symbols,
-                      dbg_philox, dbg_uniform, dbg_tnpos, dbg_norm_inv, dbg_cheng, set_option, reset_options, get_option, chol_schedule)
+                      dbg_philox, dbg_uniform, dbg_tnpos, dbg_norm_inv, dbg_cheng, set_option, reset_options, get_option, chol_schedule, xtz_noalloc,
+                      noalloc_scratch_bytes)

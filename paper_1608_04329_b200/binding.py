@@ -84,6 +84,9 @@ def lib():
     L.hsp_output_ready.argtypes = [vp, C.POINTER(ll)]
     L.hsp_output_wait.argtypes = [vp, C.POINTER(ll)]
     L.hsp_dbg_chol_trace.restype = ll
+    L.hsp_xtz_noalloc.argtypes = [vp, C.c_int, vp, ll, C.c_int, ull, ll, vp, vp, vp, vp]
+    L.hsp_noalloc_scratch_bytes.restype = ll
+    L.hsp_noalloc_last_error.restype = C.c_char_p
     L.hsp_dbg_chol_schedule.argtypes = [C.c_int, C.c_int, C.c_int, vp, ll, dp]
     L.hsp_dbg_chol_schedule.restype = ll
     _lib = L
@@ -292,6 +295,22 @@ class HorseshoeProbit:
         if n2 < 0:
             _check(int(n2))
         return rows
+
+
+def xtz_noalloc(X, y, seed, k, beta, g_out, z_out=None, stream=None):
+    """hsp_xtz_noalloc: torch CUDA tensors in, results written into the caller's g_out [p] (and z_out [N]) -- nothing is allocated."""
+    import torch
+    N, p = X.shape
+    assert X.is_contiguous() and y.dtype == torch.uint8 and beta.dtype == torch.float64 and g_out.dtype == torch.float64
+    dt = HSP_F32 if X.dtype == torch.float32 else HSP_F64
+    rc = lib().hsp_xtz_noalloc(X.data_ptr(), dt, y.data_ptr(), N, p, int(seed), int(k), beta.data_ptr(), g_out.data_ptr(),
+                               None if z_out is None else z_out.data_ptr(), _stream_handle(stream)[0])
+    if rc != HSP_OK:
+        raise HspError(rc, lib().hsp_noalloc_last_error().decode())
+
+
+def noalloc_scratch_bytes():
+    return int(lib().hsp_noalloc_scratch_bytes())
 
 
 def chol_schedule(nt, sb, K):
